@@ -1,0 +1,368 @@
+/*
+ * sf_oracle.c -- float64 CPU oracle for the SF-TR projector pair.  TEST INFRASTRUCTURE ONLY.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * build, load or call this file.  It shares no code, header, table or helper with the CUDA path
+ * under paper_2503_16741_b200/csrc/ and is never used as a fallback by the product.
+ *
+ * What it computes.  PAPER.md:93-101 (Sec. 2.3, Eq. (1) y = A x and Eq. (2) x = A^T y) with the
+ * "separable footprint (SF)" voxel model of PAPER.md:103 ("volume-based voxel model", strict
+ * adjoint).  The paper never prints the SF formulas; the step-by-step definition followed here
+ * is the reading SURVEY.md Sec. 8(c) O1-O7 / DESIGN.md "Readings" R1-R18 (trapezoid transaxial
+ * footprint x rectangular axial footprint, voxel-centre amplitude, cell-averaged response).
+ * SF-TR is an approximation, so this file follows the algorithm in that order and notation; it
+ * is written for legibility, not speed: no blocking, no fusion, no hoisting out of loops.
+ *
+ * Pins (tests/test_oracle_pins.py, -m "not gpu"): trapezoid CDF vs quadrature; hand-worked 2-D
+ * and 3-D footprints; brute-force ray/box chords; analytic disk/ellipsoid chords; mass
+ * identities; parallel-beam column sums; 2-D == one-slice 3-D; dense-matrix transpose; adjoint
+ * to 1e-12; symmetries.  Unpinned: arc detector in a tilted frame beyond brute force (R8).
+ *
+ * Build: gcc -O2 -fopenmp -shared -fPIC -o libsf_oracle.so sf_oracle.c -lm
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* Problem description (own definition; deliberately not the product's ct_geom_desc_t header). */
+typedef struct {
+    int dim;                 /* 2 or 3 */
+    int nx, ny, nz;
+    double dx, dy, dz;       /* mm */
+    double ox, oy, oz;       /* world position of the volume centre */
+    int nu, nv;
+    double du, dv;           /* mm; arc: du is arc length at radius R */
+    int det_type;            /* 0 flat, 1 arc */
+    int n_views;
+    const double *src;       /* [n_views][3] */
+    const double *det_center;/* [n_views][3] */
+    const double *det_u;     /* [n_views][3] */
+    const double *det_v;     /* [n_views][3]; dim 2: ignored, taken as (0,0,1) */
+} sfo_geom;
+
+/* O1: per-view frame. */
+typedef struct { double S[3], u[3], v[3], n[3], R, Du, Dv; } sfo_frame;
+
+static double dot3(const double *a, const double *b) { return a[0]*b[0] + a[1]*b[1] + a[2]*b[2]; }
+
+static void make_frame(const sfo_geom *g, int view, sfo_frame *f)
+{
+    const double *S = g->src + 3*view, *D = g->det_center + 3*view, *u = g->det_u + 3*view;
+    double v[3] = {0.0, 0.0, 1.0};
+    if (g->dim == 3) { v[0] = g->det_v[3*view]; v[1] = g->det_v[3*view+1]; v[2] = g->det_v[3*view+2]; }
+    double n[3] = { u[1]*v[2] - u[2]*v[1], u[2]*v[0] - u[0]*v[2], u[0]*v[1] - u[1]*v[0] };
+    double DS[3] = { D[0]-S[0], D[1]-S[1], D[2]-S[2] };
+    if (dot3(DS, n) < 0.0) { n[0] = -n[0]; n[1] = -n[1]; n[2] = -n[2]; }   /* (D-S).n > 0 */
+    for (int c = 0; c < 3; ++c) { f->S[c] = S[c]; f->u[c] = u[c]; f->v[c] = v[c]; f->n[c] = n[c]; }
+    f->R  = dot3(DS, n);
+    f->Du = dot3(DS, u);
+    f->Dv = dot3(DS, v);
+}
+
+/* Detector coordinates (s, t) in mm of a world point P (SURVEY 8 "Notation").
+ * Returns 0 if P is not in front of the source (a <= 0). */
+static int det_coords(const sfo_geom *g, const sfo_frame *f, const double *P, double *s, double *t)
+{
+    double w[3] = { P[0]-f->S[0], P[1]-f->S[1], P[2]-f->S[2] };
+    double a = dot3(w, f->n), b = dot3(w, f->u), c = dot3(w, f->v);
+    if (!(a > 0.0)) return 0;
+    if (g->det_type == 0) {            /* flat */
+        *s = f->R * b / a - f->Du;
+        *t = f->R * c / a - f->Dv;
+    } else {                           /* arc: cylinder of radius R about the line through S along v */
+        *s = f->R * atan2(b, a);
+        *t = f->R * c / sqrt(a*a + b*b) - f->Dv;
+    }
+    return 1;
+}
+
+/* O4: CDF of the unit-height trapezoid with vertices tau[0] <= tau[1] <= tau[2] <= tau[3].
+ * Half-open branches: a zero-width ramp is an empty branch, so no 0/0 is evaluated. */
+double sfo_trap_cdf(const double *tau, double s)
+{
+    const double t0 = tau[0], t1 = tau[1], t2 = tau[2], t3 = tau[3];
+    if (s <= t0) return 0.0;
+    if (s <= t1) return (s - t0)*(s - t0) / (2.0*(t1 - t0));
+    if (s <= t2) return (t1 - t0)/2.0 + (s - t1);
+    if (s <= t3) return (t1 - t0)/2.0 + (t2 - t1) + (s - t2) - (s - t2)*(s - t2) / (2.0*(t3 - t2));
+    return (t1 - t0)/2.0 + (t2 - t1) + (t3 - t2)/2.0;
+}
+
+static void sort4(double *a)
+{
+    for (int i = 1; i < 4; ++i) {
+        double x = a[i]; int j = i - 1;
+        while (j >= 0 && a[j] > x) { a[j+1] = a[j]; --j; }
+        a[j+1] = x;
+    }
+}
+
+/* O2-O6 for one (view, voxel).  Outputs the cell ranges [k_lo, k_hi], [l_lo, l_hi] (empty when
+ * lo > hi), F1[k - k_lo], F2[l - l_lo] and the amplitude.  F1 must hold nu doubles, F2 nv doubles.
+ * Returns 1 when the footprint touches the detector, 0 otherwise. */
+static int footprint(const sfo_geom *g, const sfo_frame *f, int ix, int iy, int iz,
+                     int *k_lo, int *k_hi, double *F1, int *l_lo, int *l_hi, double *F2,
+                     double *amp, double *tau_out)
+{
+    /* voxel centre (R9) */
+    double Pc[3] = { g->ox + (ix - 0.5*(g->nx - 1))*g->dx,
+                     g->oy + (iy - 0.5*(g->ny - 1))*g->dy,
+                     g->dim == 3 ? g->oz + (iz - 0.5*(g->nz - 1))*g->dz : 0.0 };
+    /* O3: transaxial corners at the voxel mid-plane (R4) */
+    double tau[4]; int c = 0;
+    for (int sx = -1; sx <= 1; sx += 2)
+        for (int sy = -1; sy <= 1; sy += 2) {
+            double P[3] = { Pc[0] + sx*0.5*g->dx, Pc[1] + sy*0.5*g->dy, Pc[2] };
+            double t_unused;
+            if (!det_coords(g, f, P, &tau[c], &t_unused)) return 0;       /* O2 */
+            ++c;
+        }
+    sort4(tau);
+    if (tau_out) memcpy(tau_out, tau, sizeof tau);
+    /* O4: transaxial cell range and cell-averaged weights (R3, R12, R15) */
+    int klo = (int)floor(tau[0]/g->du + 0.5*g->nu), khi = (int)floor(tau[3]/g->du + 0.5*g->nu);
+    if (klo < 0) klo = 0;
+    if (khi > g->nu - 1) khi = g->nu - 1;
+    *k_lo = klo; *k_hi = khi;
+    if (klo > khi) return 0;
+    for (int k = klo; k <= khi; ++k) {
+        double uk = (k - 0.5*(g->nu - 1))*g->du;
+        F1[k - klo] = (sfo_trap_cdf(tau, uk + 0.5*g->du) - sfo_trap_cdf(tau, uk - 0.5*g->du)) / g->du;
+    }
+    /* O5: axial footprint (R5) */
+    if (g->dim == 3) {
+        double Pm[3] = { Pc[0], Pc[1], Pc[2] - 0.5*g->dz }, Pp[3] = { Pc[0], Pc[1], Pc[2] + 0.5*g->dz };
+        double s_unused, ta, tb;
+        if (!det_coords(g, f, Pm, &s_unused, &ta)) return 0;
+        if (!det_coords(g, f, Pp, &s_unused, &tb)) return 0;
+        double tlo = ta < tb ? ta : tb, thi = ta < tb ? tb : ta;
+        int llo = (int)floor(tlo/g->dv + 0.5*g->nv), lhi = (int)floor(thi/g->dv + 0.5*g->nv);
+        if (llo < 0) llo = 0;
+        if (lhi > g->nv - 1) lhi = g->nv - 1;
+        *l_lo = llo; *l_hi = lhi;
+        if (llo > lhi) return 0;
+        for (int l = llo; l <= lhi; ++l) {
+            double vl = (l - 0.5*(g->nv - 1))*g->dv;
+            double hi = vl + 0.5*g->dv < thi ? vl + 0.5*g->dv : thi;
+            double lo = vl - 0.5*g->dv > tlo ? vl - 0.5*g->dv : tlo;
+            F2[l - llo] = (hi - lo > 0.0 ? hi - lo : 0.0) / g->dv;
+        }
+    } else {
+        *l_lo = 0; *l_hi = 0; F2[0] = 1.0;                                  /* R18 */
+    }
+    /* O6: amplitude along the voxel-centre ray (R2, R14) */
+    double e[3] = { Pc[0]-f->S[0], Pc[1]-f->S[1], g->dim == 3 ? Pc[2]-f->S[2] : 0.0 };
+    double norm = sqrt(e[0]*e[0] + e[1]*e[1] + e[2]*e[2]);
+    double rx = g->dx / fabs(e[0]), ry = g->dy / fabs(e[1]);                /* x/0 = +inf */
+    *amp = norm * (rx < ry ? rx : ry);
+    return 1;
+}
+
+/* ---- public entry points (all arrays double, C-contiguous) ------------------------------- */
+
+/* Footprint of one voxel in one view, for the pins.  F1 (nu doubles) and F2 (nv doubles) are
+ * caller-allocated.  rng_out = {k_lo, k_hi, l_lo, l_hi}; tau_out = 4 sorted vertices. */
+int sfo_footprint(const sfo_geom *g, int view, int ix, int iy, int iz,
+                  int *rng_out, double *F1, double *F2, double *amp, double *tau_out)
+{
+    sfo_frame f; make_frame(g, view, &f);
+    rng_out[0] = 0; rng_out[1] = -1; rng_out[2] = 0; rng_out[3] = -1;
+    return footprint(g, &f, ix, iy, iz, &rng_out[0], &rng_out[1], F1, &rng_out[2], &rng_out[3], F2, amp, tau_out);
+}
+
+/* Detector coordinates of a world point in one view (for the brute-force pins). */
+int sfo_det_coords(const sfo_geom *g, int view, const double *P, double *st)
+{
+    sfo_frame f; make_frame(g, view, &f);
+    return det_coords(g, &f, P, &st[0], &st[1]);
+}
+
+/* O7, forward: one view of y += A x restricted to slices [z0, z1). y is [nv][nu]. */
+static void fp_view_slab(const sfo_geom *g, const sfo_frame *f, const double *vol, double *y,
+                         int z0, int z1, double *F1, double *F2)
+{
+    for (int iz = z0; iz < z1; ++iz)
+        for (int iy = 0; iy < g->ny; ++iy)
+            for (int ix = 0; ix < g->nx; ++ix) {
+                double xv = vol[((size_t)iz*g->ny + iy)*g->nx + ix];
+                int klo, khi, llo, lhi; double amp;
+                if (!footprint(g, f, ix, iy, iz, &klo, &khi, F1, &llo, &lhi, F2, &amp, NULL)) continue;
+                for (int l = llo; l <= lhi; ++l)
+                    for (int k = klo; k <= khi; ++k)
+                        y[(size_t)l*g->nu + k] += amp * F1[k - klo] * F2[l - llo] * xv;
+            }
+}
+
+/* y[j] = (A x)[views[j]] for j < n_sel.  vol [nz][ny][nx]; proj [n_sel][nv][nu] (overwritten).
+ * Deterministic for a fixed thread count.  Returns the number of threads used. */
+int sfo_fp(const sfo_geom *g, const double *vol, const int *views, int n_sel, double *proj)
+{
+    const size_t ncell = (size_t)g->nu * g->nv;
+    int nthreads = 1;
+#ifdef _OPENMP
+    nthreads = omp_get_max_threads();
+#endif
+    memset(proj, 0, sizeof(double) * ncell * n_sel);
+    if (g->nz < 2*nthreads || n_sel >= 4*nthreads) {
+        /* parallel over views: every view's output is private */
+        #pragma omp parallel
+        {
+            double *F1 = malloc(sizeof(double)*g->nu), *F2 = malloc(sizeof(double)*g->nv);
+            #pragma omp for schedule(dynamic, 1)
+            for (int j = 0; j < n_sel; ++j) {
+                sfo_frame f; make_frame(g, views[j], &f);
+                fp_view_slab(g, &f, vol, proj + ncell*j, 0, g->nz, F1, F2);
+            }
+            free(F1); free(F2);
+        }
+    } else {
+        /* few views, many slices: split slices statically, private partial images, ordered sum */
+        double *part = malloc(sizeof(double) * ncell * nthreads);
+        for (int j = 0; j < n_sel; ++j) {
+            sfo_frame f; make_frame(g, views[j], &f);
+            memset(part, 0, sizeof(double) * ncell * nthreads);
+            #pragma omp parallel num_threads(nthreads)
+            {
+                int tid = 0, nt = 1;
+#ifdef _OPENMP
+                tid = omp_get_thread_num(); nt = omp_get_num_threads();
+#endif
+                double *F1 = malloc(sizeof(double)*g->nu), *F2 = malloc(sizeof(double)*g->nv);
+                int z0 = (int)((long)g->nz * tid / nt), z1 = (int)((long)g->nz * (tid+1) / nt);
+                fp_view_slab(g, &f, vol, part + ncell*tid, z0, z1, F1, F2);
+                free(F1); free(F2);
+            }
+            for (int t = 0; t < nthreads; ++t)
+                for (size_t c = 0; c < ncell; ++c) proj[ncell*j + c] += part[ncell*t + c];
+        }
+        free(part);
+    }
+    return nthreads;
+}
+
+/* O7, adjoint, one voxel: sum over the selected views in order. proj is [n_sel][nv][nu]. */
+static double bp_voxel(const sfo_geom *g, const sfo_frame *frames, const double *proj, int n_sel,
+                       int ix, int iy, int iz, double *F1, double *F2)
+{
+    const size_t ncell = (size_t)g->nu * g->nv;
+    double acc = 0.0;
+    for (int j = 0; j < n_sel; ++j) {
+        int klo, khi, llo, lhi; double amp;
+        if (!footprint(g, &frames[j], ix, iy, iz, &klo, &khi, F1, &llo, &lhi, F2, &amp, NULL)) continue;
+        const double *y = proj + ncell*j;
+        for (int l = llo; l <= lhi; ++l)
+            for (int k = klo; k <= khi; ++k)
+                acc += amp * F1[k - klo] * F2[l - llo] * y[(size_t)l*g->nu + k];
+    }
+    return acc;
+}
+
+/* vol = A^T y over the selected views.  proj [n_sel][nv][nu]; vol [nz][ny][nx] (overwritten). */
+int sfo_bp(const sfo_geom *g, const double *proj, const int *views, int n_sel, double *vol)
+{
+    int nthreads = 1;
+#ifdef _OPENMP
+    nthreads = omp_get_max_threads();
+#endif
+    sfo_frame *frames = malloc(sizeof(sfo_frame) * (n_sel > 0 ? n_sel : 1));
+    for (int j = 0; j < n_sel; ++j) make_frame(g, views[j], &frames[j]);
+    #pragma omp parallel
+    {
+        double *F1 = malloc(sizeof(double)*g->nu), *F2 = malloc(sizeof(double)*g->nv);
+        #pragma omp for schedule(dynamic, 4) collapse(2)
+        for (int iz = 0; iz < g->nz; ++iz)
+            for (int iy = 0; iy < g->ny; ++iy)
+                for (int ix = 0; ix < g->nx; ++ix)
+                    vol[((size_t)iz*g->ny + iy)*g->nx + ix] = bp_voxel(g, frames, proj, n_sel, ix, iy, iz, F1, F2);
+        free(F1); free(F2);
+    }
+    free(frames);
+    return nthreads;
+}
+
+/* (A^T y) at n listed voxels (ijk[3*i..] = ix, iy, iz), all views; y is the FULL [n_views][nv][nu]. */
+int sfo_bp_voxels(const sfo_geom *g, const double *proj, const int *ijk, int n, double *out)
+{
+    int nthreads = 1;
+#ifdef _OPENMP
+    nthreads = omp_get_max_threads();
+#endif
+    sfo_frame *frames = malloc(sizeof(sfo_frame) * g->n_views);
+    for (int j = 0; j < g->n_views; ++j) make_frame(g, j, &frames[j]);
+    #pragma omp parallel
+    {
+        double *F1 = malloc(sizeof(double)*g->nu), *F2 = malloc(sizeof(double)*g->nv);
+        #pragma omp for schedule(dynamic, 16)
+        for (int i = 0; i < n; ++i)
+            out[i] = bp_voxel(g, frames, proj, g->n_views, ijk[3*i], ijk[3*i+1], ijk[3*i+2], F1, F2);
+        free(F1); free(F2);
+    }
+    free(frames);
+    return nthreads;
+}
+
+/* Same as sfo_bp_voxels but the projections are given in float32 (the full-size config-4
+ * projection set is 1.6 GB in fp32; widening all of it to float64 would need 3.4 GB more).
+ * Each value is widened to double before use. */
+int sfo_bp_voxels_f32(const sfo_geom *g, const float *proj, const int *ijk, int n, double *out)
+{
+    int nthreads = 1;
+#ifdef _OPENMP
+    nthreads = omp_get_max_threads();
+#endif
+    const size_t ncell = (size_t)g->nu * g->nv;
+    sfo_frame *frames = malloc(sizeof(sfo_frame) * g->n_views);
+    for (int j = 0; j < g->n_views; ++j) make_frame(g, j, &frames[j]);
+    #pragma omp parallel
+    {
+        double *F1 = malloc(sizeof(double)*g->nu), *F2 = malloc(sizeof(double)*g->nv);
+        #pragma omp for schedule(dynamic, 16)
+        for (int i = 0; i < n; ++i) {
+            double acc = 0.0;
+            for (int j = 0; j < g->n_views; ++j) {
+                int klo, khi, llo, lhi; double amp;
+                if (!footprint(g, &frames[j], ijk[3*i], ijk[3*i+1], ijk[3*i+2], &klo, &khi, F1, &llo, &lhi, F2, &amp, NULL)) continue;
+                const float *y = proj + ncell*j;
+                for (int l = llo; l <= lhi; ++l)
+                    for (int k = klo; k <= khi; ++k)
+                        acc += amp * F1[k - klo] * F2[l - llo] * (double)y[(size_t)l*g->nu + k];
+            }
+            out[i] = acc;
+        }
+        free(F1); free(F2);
+    }
+    free(frames);
+    return nthreads;
+}
+
+/* Fraction of voxel x view pairs whose footprint touches the detector ("live"), on a strided
+ * sample of voxels and views; reported by the bench next to GUPS. */
+double sfo_live_fraction(const sfo_geom *g, int vox_stride, int view_stride)
+{
+    long live = 0, total = 0;
+    double *F1 = malloc(sizeof(double)*g->nu), *F2 = malloc(sizeof(double)*g->nv);
+    for (int j = 0; j < g->n_views; j += view_stride) {
+        sfo_frame f; make_frame(g, j, &f);
+        for (int iz = 0; iz < g->nz; iz += vox_stride)
+            for (int iy = 0; iy < g->ny; iy += vox_stride)
+                for (int ix = 0; ix < g->nx; ix += vox_stride) {
+                    int klo, khi, llo, lhi; double amp;
+                    live += footprint(g, &f, ix, iy, iz, &klo, &khi, F1, &llo, &lhi, F2, &amp, NULL);
+                    ++total;
+                }
+    }
+    free(F1); free(F2);
+    return total ? (double)live / (double)total : 0.0;
+}
+
+int sfo_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
