@@ -1,0 +1,117 @@
+/*
+ * ctsf.h -- C ABI of the B200-native separable-footprint (SF-TR) projector pair.
+ *
+ * The operation.  PAPER.md:93-101 (Sec. 2.3): forward projection y = A x (Eq. 1) and its exact
+ * adjoint x = A^T y (Eq. 2), a "matched" pair, with the separable-footprint voxel model of
+ * PAPER.md:103 ("volume-based voxel model", strict adjoint implemented), for the three scan
+ * geometries of PAPER.md:72 / Table 2 (2-D fan, 3-D circular, 3-D non-circular, every parameter
+ * view-specific) and flat or curved detectors.  The SF-TR arithmetic itself
+ * (trapezoid transaxial x rectangle axial footprint, voxel-centre amplitude, cell-averaged
+ * response) is spelled out in DESIGN.md "The method" with the readings R1-R18 it rests on.
+ *
+ * Conventions (all entry points):
+ *  - plain C, no torch types; pointers are HOST or DEVICE as stated per argument;
+ *  - volumes are dense fp32 [batch][nz][ny][nx], x fastest; projections are dense fp32
+ *    [batch][n_views][nv][nu], u fastest (batch = B*C flattened);
+ *  - outputs are OVERWRITTEN (y = A x, x = A^T y), never accumulated into;
+ *  - device entry points are asynchronous on `stream`: no host synchronisation, no host<->device
+ *    copy of image data; scratch memory, when needed, comes from the stream-ordered allocator;
+ *  - every function returns a ct_status_t; nothing throws across the boundary.
+ */
+#ifndef CTSF_H
+#define CTSF_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define CTSF_API __attribute__((visibility("default")))
+#else
+#define CTSF_API
+#endif
+
+typedef struct ct_geom ct_geom_t;          /* opaque; owns the device copy of the per-view parameters */
+typedef void *ct_stream_t;                 /* a cudaStream_t (0 / NULL = the legacy default stream) */
+
+typedef enum {
+    CT_OK = 0,
+    CT_ERR_INVALID_ARG = 1,   /* null pointer, non-positive size, dim==2 with nz!=1 or nv!=1, batch<1 */
+    CT_ERR_GEOMETRY = 2,      /* axes not unit/orthogonal, detector behind the source, arc detector not
+                                 centred on the source axis, volume reaching the source plane, a 2-D
+                                 geometry with out-of-plane components */
+    CT_ERR_UNSUPPORTED = 3,   /* problem too large for 32-bit indexing of one image */
+    CT_ERR_ALLOC = 4,         /* host or device allocation failed */
+    CT_ERR_CUDA = 5           /* a CUDA runtime call or kernel launch failed (no usable device, ...) */
+} ct_status_t;
+
+/* Scan description (Table 2, in vector form: one source / detector frame per view).
+ * World frame in mm.  Voxel (ix,iy,iz) is centred at (ox + (ix-(nx-1)/2) dx, oy + ..., oz + ...).
+ * Detector cell (k,l) is centred at detector coordinates u_k = (k-(nu-1)/2) du, v_l = (l-(nv-1)/2) dv,
+ * measured from det_center along det_u / det_v (flat), or as arc length du at radius R about the
+ * line through the source parallel to det_v (arc: equi-angular channels, equi-spaced rows). */
+typedef struct {
+    int32_t dim;                 /* 2 or 3.  dim==2: nz==1, nv==1, no axial factor; z components must be 0 */
+    int32_t nx, ny, nz;          /* voxels */
+    double  dx, dy, dz;          /* voxel pitch, mm (> 0) */
+    double  ox, oy, oz;          /* world position of the volume centre ("object centre") */
+    int32_t nu, nv;              /* detector channels, rows */
+    double  du, dv;              /* cell pitch, mm (> 0) */
+    int32_t det_type;            /* 0 flat, 1 arc */
+    int32_t n_views;
+    const double *src;           /* HOST [n_views][3] source position */
+    const double *det_center;    /* HOST [n_views][3] detector point with detector coordinates (0,0) */
+    const double *det_u;         /* HOST [n_views][3] unit vector along channels */
+    const double *det_v;         /* HOST [n_views][3] unit vector along rows (arc: the cylinder axis);
+                                    may be NULL when dim==2 (taken as (0,0,1)) */
+} ct_geom_desc_t;
+
+/* Validates `desc`, derives the per-view kernel parameters in float64, rounds them to fp32 and
+ * uploads them to the current CUDA device.  The host arrays are copied; the caller may free them
+ * afterwards.  *out is immutable after creation and may be used from several streams at once.
+ * Errors: CT_ERR_INVALID_ARG, CT_ERR_GEOMETRY, CT_ERR_UNSUPPORTED, CT_ERR_ALLOC, CT_ERR_CUDA. */
+CTSF_API ct_status_t ct_geom_create(const ct_geom_desc_t *desc, ct_geom_t **out);
+
+/* Frees the geometry and its device memory.  ct_geom_destroy(NULL) is CT_OK. */
+CTSF_API ct_status_t ct_geom_destroy(ct_geom_t *geom);
+
+/* y = A x (Eq. 1).  d_vol: DEVICE, read, [batch][nz][ny][nx].
+ * d_proj: DEVICE, written (every element exactly once), [batch][n_views][nv][nu].
+ * Both 16-byte aligned, caller-owned, must not overlap.  Asynchronous on `stream`. */
+CTSF_API ct_status_t ct_fp_sf(const ct_geom_t *geom, const float *d_vol, float *d_proj,
+                     int32_t batch, ct_stream_t stream);
+
+/* x = A^T y (Eq. 2): the exact transpose of the weights of ct_fp_sf.
+ * d_proj: DEVICE, read; d_vol: DEVICE, written (every element exactly once).  Asynchronous. */
+CTSF_API ct_status_t ct_bp_sf(const ct_geom_t *geom, const float *d_proj, float *d_vol,
+                     int32_t batch, ct_stream_t stream);
+
+/* Ordered-subset variants: the operators restricted to views
+ * view_begin, view_begin + view_stride, ... (view_count of them).  The projection buffer holds
+ * ONLY the selected views: [batch][view_count][nv][nu]. */
+CTSF_API ct_status_t ct_fp_sf_views(const ct_geom_t *geom, const float *d_vol, float *d_proj, int32_t batch,
+                           int32_t view_begin, int32_t view_stride, int32_t view_count, ct_stream_t stream);
+CTSF_API ct_status_t ct_bp_sf_views(const ct_geom_t *geom, const float *d_proj, float *d_vol, int32_t batch,
+                           int32_t view_begin, int32_t view_stride, int32_t view_count, ct_stream_t stream);
+
+/* End-to-end convenience with HOST buffers (pageable or pinned): allocates device buffers from the
+ * stream-ordered pool, copies the input host->device, runs the operator, copies the result
+ * device->host and synchronises `stream` before returning.  Same layouts as above. */
+CTSF_API ct_status_t ct_fp_sf_host(const ct_geom_t *geom, const float *h_vol, float *h_proj,
+                          int32_t batch, ct_stream_t stream);
+CTSF_API ct_status_t ct_bp_sf_host(const ct_geom_t *geom, const float *h_proj, float *h_vol,
+                          int32_t batch, ct_stream_t stream);
+
+/* Number of kernels the LAST ct_fp_sf / ct_bp_sf call on this geometry launched (for the bench's
+ * gpu_launches count).  Not thread-safe against concurrent calls on the same geometry. */
+CTSF_API int32_t ct_last_launch_count(const ct_geom_t *geom);
+
+/* Static description of a status code; never NULL. */
+CTSF_API const char *ct_status_string(ct_status_t status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CTSF_H */

@@ -1,0 +1,167 @@
+// ctsf_api.cu -- the C ABI of libctsf (include/ctsf.h): argument checks, geometry lifetime,
+// kernel scheduling ("C++ projector function manages kernel scheduling").
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <new>
+
+#include "ctsf_internal.h"
+
+namespace {
+
+bool finite_pos(double x) { return std::isfinite(x) && x > 0.0; }
+
+ct_status_t check_call(const ct_geom *g, const void *a, const void *b, int batch, int vb, int vs, int vc)
+{
+    if (!g || !a || !b || batch < 1) return CT_ERR_INVALID_ARG;
+    if (vc < 0 || vs < 1 || vb < 0) return CT_ERR_INVALID_ARG;
+    if (vc > 0 && (long)vb + (long)(vc - 1) * vs >= g->prob.n_views) return CT_ERR_INVALID_ARG;
+    if (((uintptr_t)a | (uintptr_t)b) & 15u) return CT_ERR_INVALID_ARG;
+    return CT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+ct_status_t ct_geom_create(const ct_geom_desc_t *d, ct_geom_t **out)
+{
+    if (!d || !out) return CT_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (d->dim != 2 && d->dim != 3) return CT_ERR_INVALID_ARG;
+    if (d->nx < 1 || d->ny < 1 || d->nz < 1 || d->nu < 1 || d->nv < 1 || d->n_views < 1) return CT_ERR_INVALID_ARG;
+    if (d->dim == 2 && (d->nz != 1 || d->nv != 1)) return CT_ERR_INVALID_ARG;
+    if (!finite_pos(d->dx) || !finite_pos(d->dy) || !finite_pos(d->du)) return CT_ERR_INVALID_ARG;
+    if (d->dim == 3 && (!finite_pos(d->dz) || !finite_pos(d->dv))) return CT_ERR_INVALID_ARG;
+    if (!std::isfinite(d->ox) || !std::isfinite(d->oy) || (d->dim == 3 && !std::isfinite(d->oz))) return CT_ERR_INVALID_ARG;
+    if (d->det_type != 0 && d->det_type != 1) return CT_ERR_INVALID_ARG;
+    if (!d->src || !d->det_center || !d->det_u || (d->dim == 3 && !d->det_v)) return CT_ERR_INVALID_ARG;
+    if ((double)d->nx * d->ny * d->nz >= 2147483648.0 || (double)d->nu * d->nv * d->n_views >= 2147483648.0 * 4)
+        return CT_ERR_UNSUPPORTED;
+    for (long i = 0; i < 3L * d->n_views; ++i)
+        if (!std::isfinite(d->src[i]) || !std::isfinite(d->det_center[i]) || !std::isfinite(d->det_u[i]) ||
+            (d->det_v && !std::isfinite(d->det_v[i])))
+            return CT_ERR_GEOMETRY;
+
+    ct_geom *g = new (std::nothrow) ct_geom;
+    if (!g) return CT_ERR_ALLOC;
+    g->prob = SfProblem{d->dim, d->det_type, d->nx, d->ny, d->nz, d->nu, d->nv, d->n_views};
+    ct_status_t st;
+    try {
+        st = ctsf_build_views(d, g);
+    } catch (const std::bad_alloc &) {
+        st = CT_ERR_ALLOC;
+    }
+    if (st != CT_OK) { delete g; return st; }
+
+    if (cudaGetDevice(&g->device) != cudaSuccess) { cudaGetLastError(); delete g; return CT_ERR_CUDA; }
+    const size_t bytes = sizeof(SfView) * (size_t)d->n_views;
+    if (cudaMalloc((void **)&g->d_bp, bytes) != cudaSuccess || cudaMalloc((void **)&g->d_fp, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        if (g->d_bp) cudaFree(g->d_bp);
+        delete g;
+        return CT_ERR_ALLOC;
+    }
+    if (cudaMemcpy(g->d_bp, g->h_bp.data(), bytes, cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(g->d_fp, g->h_fp.data(), bytes, cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError();
+        cudaFree(g->d_bp); cudaFree(g->d_fp);
+        delete g;
+        return CT_ERR_CUDA;
+    }
+    *out = g;
+    return CT_OK;
+}
+
+ct_status_t ct_geom_destroy(ct_geom_t *g)
+{
+    if (!g) return CT_OK;
+    if (g->d_bp) cudaFree(g->d_bp);
+    if (g->d_fp) cudaFree(g->d_fp);
+    delete g;
+    return CT_OK;
+}
+
+ct_status_t ct_fp_sf_views(const ct_geom_t *g, const float *d_vol, float *d_proj, int32_t batch,
+                           int32_t vb, int32_t vs, int32_t vc, ct_stream_t stream)
+{
+    ct_status_t st = check_call(g, d_vol, d_proj, batch, vb, vs, vc);
+    if (st != CT_OK) return st;
+    int n = ctsf_launch_fp(g, d_vol, d_proj, batch, vb, vs, vc, stream);
+    if (n < 0) return CT_ERR_CUDA;
+    const_cast<ct_geom *>(g)->last_launches.store(n);
+    return CT_OK;
+}
+
+ct_status_t ct_bp_sf_views(const ct_geom_t *g, const float *d_proj, float *d_vol, int32_t batch,
+                           int32_t vb, int32_t vs, int32_t vc, ct_stream_t stream)
+{
+    ct_status_t st = check_call(g, d_proj, d_vol, batch, vb, vs, vc);
+    if (st != CT_OK) return st;
+    int n = ctsf_launch_bp(g, d_proj, d_vol, batch, vb, vs, vc, stream);
+    if (n < 0) return CT_ERR_CUDA;
+    const_cast<ct_geom *>(g)->last_launches.store(n);
+    return CT_OK;
+}
+
+ct_status_t ct_fp_sf(const ct_geom_t *g, const float *d_vol, float *d_proj, int32_t batch, ct_stream_t stream)
+{
+    if (!g) return CT_ERR_INVALID_ARG;
+    return ct_fp_sf_views(g, d_vol, d_proj, batch, 0, 1, g->prob.n_views, stream);
+}
+
+ct_status_t ct_bp_sf(const ct_geom_t *g, const float *d_proj, float *d_vol, int32_t batch, ct_stream_t stream)
+{
+    if (!g) return CT_ERR_INVALID_ARG;
+    return ct_bp_sf_views(g, d_proj, d_vol, batch, 0, 1, g->prob.n_views, stream);
+}
+
+static ct_status_t host_op(const ct_geom_t *g, const float *h_in, float *h_out, int32_t batch, ct_stream_t stream, bool fwd)
+{
+    if (!g || !h_in || !h_out || batch < 1) return CT_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const SfProblem &pr = g->prob;
+    const size_t nvol = (size_t)batch * pr.nx * pr.ny * pr.nz, nproj = (size_t)batch * pr.n_views * pr.nv * pr.nu;
+    const size_t n_in = fwd ? nvol : nproj, n_out = fwd ? nproj : nvol;
+    float *d_in = nullptr, *d_out = nullptr;
+    if (cudaMallocAsync((void **)&d_in, n_in * sizeof(float), st) != cudaSuccess) { cudaGetLastError(); return CT_ERR_ALLOC; }
+    if (cudaMallocAsync((void **)&d_out, n_out * sizeof(float), st) != cudaSuccess) {
+        cudaGetLastError(); cudaFreeAsync(d_in, st); return CT_ERR_ALLOC;
+    }
+    ct_status_t rc = CT_OK;
+    if (cudaMemcpyAsync(d_in, h_in, n_in * sizeof(float), cudaMemcpyHostToDevice, st) != cudaSuccess) rc = CT_ERR_CUDA;
+    if (rc == CT_OK) rc = fwd ? ct_fp_sf(g, d_in, d_out, batch, stream) : ct_bp_sf(g, d_in, d_out, batch, stream);
+    if (rc == CT_OK && cudaMemcpyAsync(h_out, d_out, n_out * sizeof(float), cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = CT_ERR_CUDA;
+    cudaFreeAsync(d_in, st);
+    cudaFreeAsync(d_out, st);
+    if (cudaStreamSynchronize(st) != cudaSuccess && rc == CT_OK) rc = CT_ERR_CUDA;
+    if (rc != CT_OK) cudaGetLastError();
+    return rc;
+}
+
+ct_status_t ct_fp_sf_host(const ct_geom_t *g, const float *h_vol, float *h_proj, int32_t batch, ct_stream_t stream)
+{
+    return host_op(g, h_vol, h_proj, batch, stream, true);
+}
+
+ct_status_t ct_bp_sf_host(const ct_geom_t *g, const float *h_proj, float *h_vol, int32_t batch, ct_stream_t stream)
+{
+    return host_op(g, h_proj, h_vol, batch, stream, false);
+}
+
+int32_t ct_last_launch_count(const ct_geom_t *g) { return g ? g->last_launches.load() : 0; }
+
+const char *ct_status_string(ct_status_t s)
+{
+    switch (s) {
+        case CT_OK: return "CT_OK";
+        case CT_ERR_INVALID_ARG: return "CT_ERR_INVALID_ARG: null pointer, bad size, misaligned buffer or bad view range";
+        case CT_ERR_GEOMETRY: return "CT_ERR_GEOMETRY: inconsistent scan geometry";
+        case CT_ERR_UNSUPPORTED: return "CT_ERR_UNSUPPORTED: problem too large";
+        case CT_ERR_ALLOC: return "CT_ERR_ALLOC: allocation failed";
+        case CT_ERR_CUDA: return "CT_ERR_CUDA: CUDA runtime error";
+    }
+    return "unknown ct_status_t";
+}
+
+}  // extern "C"

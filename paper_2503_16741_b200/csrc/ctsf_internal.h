@@ -1,0 +1,27 @@
+// ctsf_internal.h -- private declarations shared by the translation units of libctsf.
+#pragma once
+#include <atomic>
+#include <vector>
+
+#include "../../include/ctsf.h"
+#include "sf_params.h"
+
+struct ct_geom {
+    SfProblem prob;
+    std::vector<SfView> h_bp, h_fp;   // host copies (natural order / forward order with xy swaps)
+    SfView *d_bp = nullptr, *d_fp = nullptr;
+    int any_swap = 0;                 // some forward view reads the volume through its transpose
+    int all_untilted = 0;             // every view: transaxial footprint independent of z
+    int device = 0;
+    std::atomic<int> last_launches{0};
+};
+
+// geom.cpp
+ct_status_t ctsf_build_views(const ct_geom_desc_t *desc, ct_geom *g);
+
+// sf_bp.cu / sf_fp.cu: launchers.  Projection buffers hold `view_count` views; view j of the buffer
+// is geometry view view_begin + j*view_stride.  Return the number of kernels launched, or -1.
+int ctsf_launch_bp(const ct_geom *g, const float *d_proj, float *d_vol, int batch,
+                   int view_begin, int view_stride, int view_count, void *stream);
+int ctsf_launch_fp(const ct_geom *g, const float *d_vol, float *d_proj, int batch,
+                   int view_begin, int view_stride, int view_count, void *stream);
