@@ -166,3 +166,27 @@ def geom_keys(c):
 def n_updates(c):
     """Voxel x view updates of one operator application (the GUPS numerator)."""
     return c["batch"] * c["nx"] * c["ny"] * c["nz"] * c["n_views"]
+
+
+def make_projections(c, seed=None, batch=None):
+    """Smooth, positive, seeded projection-domain input for A^T at sizes where the oracle cannot
+    produce A x in reasonable time: float32 [batch, n_views, nv, nu].  A sum of three low-frequency
+    separable cosine products over (view, row, channel) on a positive offset -- sinogram-like in range
+    and smoothness, but not derived from any projector."""
+    rng = np.random.default_rng((c["seed"] if seed is None else seed) + 5000)
+    B = c["batch"] if batch is None else batch
+    nvw, nv, nu = c["n_views"], c["nv"], c["nu"]
+    out = np.empty((B, nvw, nv, nu), dtype=np.float32)
+    i = np.arange(nvw, dtype=np.float64)[:, None, None] / nvw
+    l = (np.arange(nv, dtype=np.float64)[None, :, None] + 0.5) / nv
+    k = (np.arange(nu, dtype=np.float64)[None, None, :] + 0.5) / nu
+    for b in range(B):
+        acc = np.full((nvw, nv, nu), 2.0)
+        for _ in range(3):
+            fi, fl, fk = rng.integers(1, 4), rng.integers(1, 4), rng.integers(1, 6)
+            pi_, pl, pk = rng.uniform(0, 2 * math.pi, 3)
+            amp = rng.uniform(0.2, 0.6)
+            acc = acc + amp * (np.cos(2 * math.pi * fi * i + pi_) * np.cos(math.pi * fl * l + pl)
+                               * np.cos(math.pi * fk * k + pk))
+        out[b] = acc.astype(np.float32)
+    return out

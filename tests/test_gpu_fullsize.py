@@ -1,0 +1,59 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times.
+
+The oracle cannot produce whole outputs at these sizes in reasonable time, so it computes sampled
+outputs one by one: A on a few whole views (every cell of those views is compared), A^T on randomly
+sampled voxels over all views.  Inputs: the seeded phantom (A) and a seeded smooth positive
+projection field (A^T) from the workloads module -- never anything computed by the CUDA path."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle.sf_oracle import Oracle
+from paper_2503_16741_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+N_VIEWS = {1: 6, 2: 3, 3: 3, 4: 2, 5: 4}
+N_VOX = {1: 4000, 2: 3000, 3: 3000, 4: 3000, 5: 3000}
+
+
+@pytest.mark.parametrize("index", [1, 5, 2, 3, 4])
+def test_parity_full_size_sampled(index):
+    from paper_2503_16741_b200.projector import Geometry
+    c = W.make_config(index)
+    g = W.geom_keys(c)
+    o = Oracle(g)
+    rng = np.random.default_rng(9000 + index)
+    x = W.make_phantom(c)
+    geom = Geometry(g)
+    # ---- A: whole sampled views -------------------------------------------------------------
+    xd = torch.from_numpy(x).cuda()
+    y = geom.fp(xd)                                              # full operator, as bench.py runs it
+    views = np.sort(rng.choice(c["n_views"], N_VIEWS[index], replace=False))
+    views[0] = 0 if index != 4 else views[0]
+    y_ref = o.fp(x, views)                                       # [B, n_sel, nv, nu] float64
+    y_gpu = y[:, torch.from_numpy(views).cuda()].double().cpu().numpy()
+    rel = np.linalg.norm(y_gpu - y_ref) / np.linalg.norm(y_ref)
+    mx = np.abs(y_gpu - y_ref).max() / np.abs(y_ref).max()
+    assert rel <= 1e-5 and mx <= 1e-4, "A config %d: rel-L2 %.3e max %.3e" % (index, rel, mx)
+    # every output element is written (overwrite semantics): poison the buffer first
+    y.fill_(float("nan"))
+    geom.fp(xd, out=y)
+    assert not torch.isnan(y).any()
+    del y, xd
+    # ---- A^T: sampled voxels over all views -----------------------------------------------
+    p = W.make_projections(c)
+    pd = torch.from_numpy(p).cuda()
+    xb = geom.bp(pd)
+    ijk = np.stack([rng.integers(0, c["nx"], N_VOX[index]), rng.integers(0, c["ny"], N_VOX[index]),
+                    rng.integers(0, c["nz"], N_VOX[index])], axis=1)
+    ijk[0] = (0, 0, 0)
+    ijk[1] = (c["nx"] - 1, c["ny"] - 1, c["nz"] - 1)
+    for b in range(min(c["batch"], 2)):
+        ref = o.bp_voxels(p[b], ijk)
+        got = xb[b, ijk[:, 2], ijk[:, 1], ijk[:, 0]].double().cpu().numpy()
+        rel = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+        mx = np.abs(got - ref).max() / np.abs(ref).max()
+        assert rel <= 1e-5 and mx <= 1e-4, "A^T config %d: rel-L2 %.3e max %.3e" % (index, rel, mx)
+    geom.close()
