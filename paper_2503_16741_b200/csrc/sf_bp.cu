@@ -185,13 +185,21 @@ __device__ __forceinline__ float gather_tile(const float *__restrict__ tile, con
 {
     float sum = 0.0f;
     for (int lb = l_lo; lb <= l_hi; lb += LM) {
+        // rows past l_hi get weight 0 by themselves (x >= thi), rows past the tile read the zero pad rows
+        const float x0 = (float)lb - A.lc;
         float f2[LM];
 #pragma unroll
-        for (int j = 0; j < LM; ++j) f2[j] = (lb + j <= l_hi) ? sf_F2(A, (float)(lb + j)) : 0.0f;
+        for (int j = 0; j < LM; ++j) {
+            const float x = x0 + (float)j;
+            f2[j] = fmaxf(fminf(x + 1.0f, A.thi) - fmaxf(x, A.tlo), 0.0f);
+        }
         const float *row = tile + (lb - tl0) * TW + (k_lo - tk0);
-        float g0 = sf_G(T, (float)k_lo - T.kc);
+        float xi = (float)k_lo - T.kc;
+        float g0 = sf_G(T, xi);
+#pragma unroll 1
         for (int k = k_lo; k <= k_hi; ++k) {
-            const float g1 = sf_G(T, (float)(k + 1) - T.kc);
+            xi += 1.0f;
+            const float g1 = sf_G(T, xi);
             float s = 0.0f;
 #pragma unroll
             for (int j = 0; j < LM; ++j) s = fmaf(f2[j], row[j * TW], s);
@@ -204,7 +212,7 @@ __device__ __forceinline__ float gather_tile(const float *__restrict__ tile, con
 }
 
 template <int ARC>
-__global__ void __launch_bounds__(BRICK_THREADS)
+__global__ void __launch_bounds__(BRICK_THREADS, 3)
 bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ proj,
                 const __grid_constant__ CUtensorMap tmap, int use_tma, float *__restrict__ vol,
                 int view_begin, int view_stride, int view_count, int nbz)
