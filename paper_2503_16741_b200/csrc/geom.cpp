@@ -145,7 +145,7 @@ ct_status_t ctsf_build_views(const ct_geom_desc_t *d, ct_geom *g)
             // bounds over the part of the volume that projects on or near the detector
             const int np = sw ? d->ny : d->nx, nq = sw ? d->nx : d->ny, nz = is3 ? d->nz : 1;
             const int NS = 9;
-            double gp_min = 1e300, lz_min = 1e300, gz_max = 0, lp_max = 0, wk_max = 0, wl_max = 0, hk_max = 0, hl_max = 0;
+            double gp_min = 1e300, hk_max = 0, hl_max = 0;
             int used = 0;
             for (int sz = 0; sz < (is3 ? NS : 1); ++sz) for (int sq = 0; sq < NS; ++sq) for (int sp = 0; sp < NS; ++sp) {
                 double p = (np - 1) * sp / double(NS - 1), q = (nq - 1) * sq / double(NS - 1);
@@ -157,40 +157,28 @@ ct_status_t ctsf_build_views(const ct_geom_desc_t *d, ct_geom *g)
                 ++used;
                 double k1, k2, l1, l2;
                 m.project(p + 0.5, q, z, k1, l1); m.project(p - 0.5, q, z, k2, l2);
-                gp_min = std::min(gp_min, std::fabs(k1 - k2)); lp_max = std::max(lp_max, std::fabs(l1 - l2));
+                gp_min = std::min(gp_min, std::fabs(k1 - k2));
                 double klo = 1e300, khi = -1e300;
                 for (int s1 = -1; s1 <= 1; s1 += 2) for (int s2 = -1; s2 <= 1; s2 += 2) {
                     m.project(p + 0.5 * s1, q + 0.5 * s2, z, k1, l1);
                     klo = std::min(klo, k1); khi = std::max(khi, k1);
                 }
-                wk_max = std::max(wk_max, khi - klo);
                 hk_max = std::max(hk_max, std::max(khi - kc, kc - klo));
                 if (is3) {
                     m.project(p, q, z + 0.5, k1, l1); m.project(p, q, z - 0.5, k2, l2);
-                    gz_max = std::max(gz_max, std::fabs(k1 - k2)); lz_min = std::min(lz_min, std::fabs(l1 - l2));
-                    wl_max = std::max(wl_max, std::fabs(l1 - l2));
                     hl_max = std::max(hl_max, std::max(std::fabs(l1 - lc), std::fabs(l2 - lc)));
                 }
             }
-            int col_p = np, col_z = nz;
+            // lane stride of the forward kernel: voxels p and p + stride must project >= 1 cell apart
+            // (the kernel re-checks at run time and serialises if the bound is ever violated)
+            int stride = 1;
             if (used > 0) {
-                const double mg = 1.10;       // margin for variation between samples
-                const double gp = gp_min / mg, lz = is3 ? lz_min / mg : 1.0;
-                const double wk = wk_max * mg + 1.0 + 0.05, wl = is3 ? wl_max * mg + 1.0 + 0.05 : 0.0;
-                const double gz = gz_max * mg, lp = lp_max * mg;
-                int cp_ = 1, cz_ = 1;
-                for (int it = 0; it < 64; ++it) {
-                    int ncp = gp > 1e-9 ? (int)std::min<double>(np, std::ceil((wk + cz_ * gz) / gp)) : np;
-                    int ncz = is3 ? (lz > 1e-9 ? (int)std::min<double>(nz, std::ceil((wl + ncp * lp) / lz)) : nz) : 1;
-                    ncp = std::max(ncp, 1); ncz = std::max(ncz, 1);
-                    if (ncp == cp_ && ncz == cz_) break;
-                    cp_ = std::max(cp_, ncp); cz_ = std::max(cz_, ncz);
-                }
-                col_p = std::min(cp_, np); col_z = std::min(cz_, nz);
+                const double gp = gp_min / 1.10;           // margin for variation between samples
+                stride = gp > 1e-6 ? (int)std::min<double>(np, std::ceil(1.02 / gp)) : np;
             } else {
                 hk_max = 1.0; hl_max = 1.0;      // nothing of this view reaches the detector
             }
-            o.col_p = std::max(col_p, 1); o.col_z = std::max(col_z, 1);
+            o.lane_stride = std::max(stride, 1);
             o.ek = (float)(hk_max * 1.10 + 0.05);
             o.el = (float)(is3 ? hl_max * 1.10 + 0.05 : 0.0);
             g->h_fp[i] = o;

@@ -1,23 +1,21 @@
 // sf_fp.cu -- ct_fp_sf: SF-TR forward projector y = A x (Eq. 1).
 //
-// Output-exclusive design, no atomics of any kind.  One CTA owns one detector tile (TK x TL cells)
-// of one view and keeps it in shared memory for the whole pass.  It walks the voxel slabs
-// perpendicular to the view's dominant ray axis; per slab it inverse-projects the (expanded) tile
-// onto the slab to find the voxels that can touch it, and adds their footprints into the tile in
-// "colour" phases: voxels of one phase lie on a lattice (col_p, col_z) coarse enough that their
-// footprints are pairwise disjoint (bounds derived in geom.cpp), so the plain read-modify-writes
-// of a phase never collide and the summation order is fixed.  Each detector cell is stored once.
+// Output-exclusive design, no atomics of any kind.  One WARP owns one detector tile of one view and
+// keeps it in shared memory for the whole pass.  It walks the voxel slabs perpendicular to the view's
+// dominant ray axis; per slab it inverse-projects the (expanded) tile onto the slab to find the voxels
+// that can touch it, and adds their footprints into the tile in conflict-free "rounds" (see
+// fp_band_kernel).  Each detector cell is stored exactly once; the summation order is fixed.
 //
 // Views whose rays run mostly along x read the volume through an xy-transposed copy so that the
 // in-slab index p is always the memory-fastest one.
 #include <cuda_runtime.h>
 
+#include <climits>
+
 #include "ctsf_internal.h"
 #include "sf_footprint.cuh"
 
 namespace {
-
-constexpr int FP_THREADS = 256;
 
 __global__ void transpose_xy_kernel(const float *__restrict__ src, float *__restrict__ dst, int nx, int ny)
 {
@@ -54,135 +52,238 @@ __device__ __forceinline__ Ray tile_ray(const SfView &v, float kf, float lf)
     return r;
 }
 
-// tile: [NB][TL][TK] floats in dynamic shared memory
-template <int DIM, int ARC, int NB>
-__global__ void __launch_bounds__(FP_THREADS)
-fp_tile_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ vol,
-               const float *__restrict__ volT, float *__restrict__ proj, int view_begin, int view_stride,
-               int TK, int TL, int tiles_k, size_t vol_bstride, size_t proj_bstride)
-{
-    extern __shared__ float tile[];
-    __shared__ SfView sview;
-    __shared__ Ray rays[6];
-    const int tid = threadIdx.x;
-    const int jview = blockIdx.y;
-    const int tk = blockIdx.x % tiles_k, tl = blockIdx.x / tiles_k;
-    const int k0 = tk * TK, l0 = tl * TL;
-    const int tkw = min(TK, pr.nu - k0), tlh = min(TL, pr.nv - l0);
-    const int b0 = blockIdx.z * NB;
+// ---------------------------------------------------------------------------------------------------
+// warp-band forward projector
+// ---------------------------------------------------------------------------------------------------
+// One WARP owns one detector tile of one view: FTK cells x FTL rows (3-D) or FTK cells x NB images
+// (2-D), held in the warp's private slice of shared memory for the whole pass.  No block barrier is
+// ever executed.  Per slab the warp inverse-projects its (expanded) tile to a voxel rectangle and
+// sweeps it row by row: lane i takes voxel p = p_lo + i*sp (+ colour c < sp), computes its footprint
+// once, and the warp adds the footprints into the tile in K "rounds": in round j every lane updates
+// column k_lo(i) + j of its own footprint (all its rows).  k_lo is strictly monotone along the lanes
+// (sp is chosen on the host so that neighbouring lanes' voxels project >= 1 cell apart, and the
+// kernel verifies it with a warp match), so within a round the lanes touch pairwise different
+// columns; rounds are separated by __syncwarp().  Summation order is fixed => deterministic.
+constexpr int FPW = 8;            // warps per CTA
+constexpr int FTK = 64;           // cells per warp tile
+constexpr int FTL = 32;           // rows per warp tile (3-D)
+constexpr int FLM = 4;            // pad rows: the first FLM footprint rows are updated unconditionally
+constexpr unsigned FULL = 0xffffffffu;
 
-    for (int w = tid; w < (int)(sizeof(SfView) / 4); w += FP_THREADS)
-        reinterpret_cast<uint32_t *>(&sview)[w] =
+template <int DIM, int ARC, int NB>
+__global__ void __launch_bounds__(32 * FPW)
+fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ vol,
+               const float *__restrict__ volT, float *__restrict__ proj, int view_begin, int view_stride,
+               int tiles_k, int bands_l, int n_items, size_t vol_bstride, size_t proj_bstride)
+{
+    constexpr int ROWS = DIM == 3 ? FTL + FLM : NB;
+    extern __shared__ float smem[];
+    __shared__ SfView sviews[FPW];
+    __shared__ Ray srays[FPW][6];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int item = blockIdx.x * FPW + warp;
+    if (item >= n_items) return;                     // warps are independent: no block barrier below
+    const int per_view = tiles_k * bands_l;
+    const int jview = item / per_view, rem = item - jview * per_view;
+    const int bl = rem / tiles_k, tk = rem - bl * tiles_k;
+    const int k0 = tk * FTK, l0 = bl * FTL;
+    const int tkw = min(FTK, pr.nu - k0), tlh = DIM == 3 ? min(FTL, pr.nv - l0) : 1;
+    const int b0 = blockIdx.y * NB;
+    float *tile = smem + warp * (ROWS * FTK);
+
+    for (int w = lane; w < (int)(sizeof(SfView) / 4); w += 32)
+        reinterpret_cast<uint32_t *>(&sviews[warp])[w] =
             reinterpret_cast<const uint32_t *>(views + view_begin + (size_t)jview * view_stride)[w];
-    for (int i = tid; i < NB * TL * TK; i += FP_THREADS) tile[i] = 0.0f;
-    __syncthreads();
-    const SfView &v = sview;
-    if (tid < 6) {
+    for (int i = lane; i < ROWS * FTK; i += 32) tile[i] = 0.0f;
+    __syncwarp();
+    const SfView &v = sviews[warp];
+    if (lane < 6) {
         // expanded tile: corners (and, for the arc, the mid column: the slab image of an arc tile bulges)
         const float kA = (float)k0 - v.ek, kB = (float)(k0 + tkw) + v.ek;
         const float lA = (float)l0 - v.el, lB = (float)(l0 + tlh) + v.el;
-        const float kk = (tid % 3 == 0) ? kA : (tid % 3 == 1 ? kB : 0.5f * (kA + kB));
-        rays[tid] = tile_ray<ARC>(v, kk, tid < 3 ? lA : lB);
+        const float kk = (lane % 3 == 0) ? kA : (lane % 3 == 1 ? kB : 0.5f * (kA + kB));
+        srays[warp][lane] = tile_ray<ARC>(v, kk, lane < 3 ? lA : lB);
     }
-    __syncthreads();
+    __syncwarp();
 
     const int np = v.swap_xy ? pr.ny : pr.nx, nq = v.swap_xy ? pr.nx : pr.ny, nz = pr.nz;
     const float *src = (v.swap_xy ? volT : vol) + (size_t)b0 * vol_bstride;
-    const int col_p = v.col_p, col_z = DIM == 3 ? v.col_z : 1;
+    const int sp = max(1, v.lane_stride);
+    const int k_top = k0 + tkw - 1, l_top = l0 + tlh - 1;
 
     for (int iq = 0; iq < nq; ++iq) {
-        // ---- voxel region of this slab that can touch the tile (identical in every thread) -------
-        float pmin = 1e30f, pmax = -1e30f, zmin = 1e30f, zmax = -1e30f;
+        // ---- voxel region of this slab that can touch the tile (warp-uniform) --------------------
+        // The tile's frustum cuts the slab in a quadrilateral whose rows are skewed (the row coordinate
+        // depends on depth, hence on p): the region is swept in sheared coordinates (p, z' = z - shift(p)).
+        float pr_[6], zr_[6];
+        float pmin = 1e30f, pmax = -1e30f;
         bool whole = false;
         const float dqc = (float)iq - v.Sq;
 #pragma unroll
         for (int r = 0; r < 6; ++r) {
             if (DIM == 2 && r >= 3) break;
-            const Ray ry = rays[r];
+            const Ray ry = srays[warp][r];
             if (!(ry.dq * dqc > 0.0f) || fabsf(ry.dq) < 1e-3f * (fabsf(ry.dp) + fabsf(ry.dz))) whole = true;
-            const float lam = dqc / ry.dq;
-            const float pp = fmaf(lam, ry.dp, v.Sp), zz = fmaf(lam, ry.dz, v.Sz);
-            pmin = fminf(pmin, pp); pmax = fmaxf(pmax, pp);
-            zmin = fminf(zmin, zz); zmax = fmaxf(zmax, zz);
+            const float lam = dqc * rcp_nr(ry.dq);
+            pr_[r] = fmaf(lam, ry.dp, v.Sp); zr_[r] = fmaf(lam, ry.dz, v.Sz);
+            pmin = fminf(pmin, pr_[r]); pmax = fmaxf(pmax, pr_[r]);
         }
-        int p_lo = 0, p_hi = np - 1, z_lo = 0, z_hi = nz - 1;
+        int p_lo = 0, p_hi = np - 1, zs_lo = 0, zs_hi = nz - 1;
+        float sigma = 0.0f;
         if (!whole) {
             p_lo = max(0, (int)ceilf(pmin - 0.3f)); p_hi = min(np - 1, (int)floorf(pmax + 0.3f));
-            if (DIM == 3) { z_lo = max(0, (int)ceilf(zmin - 0.3f)); z_hi = min(nz - 1, (int)floorf(zmax + 0.3f)); }
+            if (DIM == 3) {
+                // mean slope dz/dp of the two tile edges l = const (rays 0,1 and 3,4)
+                const float dpp = (pr_[1] - pr_[0]) + (pr_[4] - pr_[3]);
+                const float dzz = (zr_[1] - zr_[0]) + (zr_[4] - zr_[3]);
+                sigma = fabsf(dpp) > 1.0f ? dzz / dpp : 0.0f;
+                float zmin = 1e30f, zmax = -1e30f;
+#pragma unroll
+                for (int r = 0; r < 6; ++r) {
+                    const float zs = fmaf(-sigma, pr_[r] - (float)p_lo, zr_[r]);
+                    zmin = fminf(zmin, zs); zmax = fmaxf(zmax, zs);
+                }
+                const float smax = sigma * (float)(p_hi - p_lo);           // shift range over the region
+                zs_lo = max((int)ceilf(zmin - 0.8f), -(int)ceilf(fmaxf(smax, 0.0f)) - 1);
+                zs_hi = min((int)floorf(zmax + 0.8f), nz + (int)ceilf(fmaxf(-smax, 0.0f)));
+            }
         }
-        if (p_lo > p_hi || z_lo > z_hi) continue;
-        const int npr = p_hi - p_lo + 1, nzr = z_hi - z_lo + 1;
+        if (p_lo > p_hi || zs_lo > zs_hi) continue;
+        const int npr = p_hi - p_lo + 1, nrows = zs_hi - zs_lo + 1;
         const float q = (float)iq;
         const float aq0 = fmaf(q, v.aq, v.a0), bq0 = fmaf(q, v.bq, v.b0), cq0 = fmaf(q, v.cq, v.c0);
         const float *slab = src + (size_t)iq * np;
 
-        for (int cz_i = 0; cz_i < col_z; ++cz_i) {
-            if (cz_i >= nzr) break;
-            const int cnt_z = (nzr - cz_i + col_z - 1) / col_z;
-            for (int cp_i = 0; cp_i < col_p; ++cp_i) {
-                if (cp_i >= npr) break;
-                const int cnt_p = (npr - cp_i + col_p - 1) / col_p;
-                const int cnt = cnt_p * cnt_z;
-                for (int t = tid; t < cnt; t += FP_THREADS) {
-                    const int zi = t / cnt_p, pi = t - zi * cnt_p;
-                    const int ip = p_lo + cp_i + pi * col_p, iz = z_lo + cz_i + zi * col_z;
-                    const float p = (float)ip, z = (float)iz;
-                    const float a = fmaf(z, v.az, fmaf(p, v.ap, aq0));
-                    const float b = fmaf(z, v.bz, fmaf(p, v.bp, bq0));
-                    const float c = DIM == 3 ? fmaf(z, v.cz, fmaf(p, v.cp, cq0)) : 0.0f;
-                    const float inv_a = rcp_nr(a);
-                    SfTrans T;
-                    sf_transaxial<ARC>(v, a, b, inv_a, T);
-                    const int k_lo = max(k0, (int)floorf(T.kc + T.t0));
-                    const int k_hi = min(k0 + tkw - 1, (int)floorf(T.kc + T.t3));
-                    if (k_lo > k_hi) continue;
-                    SfAxial A;
-                    int l_lo = 0, l_hi = 0;
-                    if (DIM == 3) {
-                        sf_axial<ARC>(v, a, b, c, inv_a, A);
-                        l_lo = max(l0, (int)floorf(A.lc + A.tlo));
-                        l_hi = min(l0 + tlh - 1, (int)floorf(A.lc + A.thi));
-                        if (l_lo > l_hi) continue;
-                    }
-                    const float amp = sf_amplitude(v, a, b, c, p, q);
-                    float xv[NB];
-                    const float *xp = slab + (size_t)iz * np * nq + ip;
+        for (int col = 0; col < sp; ++col) {
+            const int nprc = (npr - col + sp - 1) / sp;
+            if (nprc <= 0) break;
+            // flattened (row, pi) sweep, 32 consecutive entries per pass.  Rows are visited in the order
+            // 0, H, 1, H+1, ... so that the (at most two) voxels of equal p that can share a pass lie H
+            // rows apart and touch different detector rows; the pass verifies this before its rounds.
+            const bool multi = DIM == 3 && nrows >= 6;
+            const int rs = multi ? max(nprc, 16) : max(nprc, 32);
+            const int total = DIM == 3 ? nrows * rs : nprc;
+            const int H = (nrows + 1) >> 1;
+            int row = 0, pi = lane;
+            while (pi >= rs) { pi -= rs; ++row; }
+            for (int f0 = 0; f0 < total; f0 += 32) {
+                const int ipr = p_lo + col + sp * pi;
+                const int sh = DIM == 3 ? __float2int_rn(sigma * (float)(ipr - p_lo)) : 0;
+                const int zrow = multi ? ((row & 1) ? H + (row >> 1) : (row >> 1)) : row;
+                const int izr = DIM == 3 ? zs_lo + zrow + sh : 0;
+                const bool act = pi < nprc && row < nrows && izr >= 0 && izr < nz;
+                const int ip = act ? ipr : p_lo, iz = act ? izr : 0;
+                // advance to the next pass
+                pi += 32;
+                while (pi >= rs) { pi -= rs; ++row; }
+                const float p = (float)ip, z = (float)iz;
+                float xv[NB];
+                const float *xp = slab + (size_t)iz * np * nq + ip;
 #pragma unroll
-                    for (int bb = 0; bb < NB; ++bb) xv[bb] = amp * __ldg(xp + bb * vol_bstride);
-                    float g0 = sf_G(T, (float)k_lo - T.kc);
-                    for (int k = k_lo; k <= k_hi; ++k) {
-                        const float g1 = sf_G(T, (float)(k + 1) - T.kc);
-                        const float f1 = g1 - g0;
-                        g0 = g1;
-                        float *tc = tile + (k - k0);
+                for (int bb = 0; bb < NB; ++bb) xv[bb] = __ldg(xp + bb * vol_bstride);
+                const float a = fmaf(p, v.ap, fmaf(z, v.az, aq0)), b = fmaf(p, v.bp, fmaf(z, v.bz, bq0));
+                const float c = DIM == 3 ? fmaf(p, v.cp, fmaf(z, v.cz, cq0)) : 0.0f;
+                const float inv_a = rcp_nr(a);
+                SfTrans T;
+                sf_transaxial<ARC>(v, a, b, inv_a, T);
+                // unclipped column range: rounds are aligned on it, columns off the tile are skipped
+                const int k_lo = (int)floorf(T.kc + T.t0);
+                const int k_hi = (int)floorf(T.kc + T.t3);
+                SfAxial A;
+                int l_lo = 0, l_hi = 0;
+                if (DIM == 3) {
+                    sf_axial<ARC>(v, a, b, c, inv_a, A);
+                    l_lo = max(l0, (int)floorf(A.lc + A.tlo));
+                    l_hi = min(l_top, (int)floorf(A.lc + A.thi));
+                }
+                const bool live = act && k_hi >= k0 && k_lo <= k_top && l_lo <= l_hi;
+                // rounds j_a .. j_b of this lane update columns k_lo + j that lie on the tile
+                const int j_a = live ? max(0, k0 - k_lo) : 0;
+                const int j_b = live ? min(k_hi, k_top) - k_lo : -1;
+                const int L = live ? l_hi - l_lo + 1 : 0;
+                const int Kmax = __reduce_max_sync(FULL, j_b + 1);
+                if (Kmax == 0) continue;
+                const int Lmax = DIM == 3 ? __reduce_max_sync(FULL, L) : 1;
+                // conflict freedom of a round: live lanes have pairwise different k_lo, or (one partner at
+                // most) touch disjoint rows.  A lane touches rows l_lo .. max(l_hi, l_lo + FLM - 1).
+                const unsigned same = __match_any_sync(FULL, live ? k_lo : INT_MIN + lane) & ~(1u << lane);
+                bool fine = true;
+                if (DIM == 3) {
+                    const int partner = same ? __ffs(same) - 1 : lane;
+                    const int my_hi = max(l_hi, l_lo + FLM - 1);
+                    const int o_lo = __shfl_sync(FULL, l_lo, partner), o_hi = __shfl_sync(FULL, my_hi, partner);
+                    fine = same == 0u || (__popc(same) == 1 && (o_lo > my_hi || o_hi < l_lo));
+                } else {
+                    fine = same == 0u;
+                }
+                const bool ok = __all_sync(FULL, fine);
+                const float amp = sf_amplitude(v, a, b, c, p, q);
+#pragma unroll
+                for (int bb = 0; bb < NB; ++bb) xv[bb] *= amp;
+                float *base = tile + (live ? (DIM == 3 ? (l_lo - l0) * FTK : 0) + (k_lo - k0) : 0);
+                const float xi0 = (float)(k_lo + j_a) - T.kc;
+                const int n_serial = ok ? 1 : 32;       // !ok: one lane at a time (never expected)
+                for (int ser = 0; ser < n_serial; ++ser) {
+                    const int jb = (ok || lane == ser) ? j_b : -1;
+                    for (int lb = 0; lb < Lmax; lb += 2 * FLM) {
+                        float f2[2 * FLM];
                         if (DIM == 3) {
-                            for (int l = l_lo; l <= l_hi; ++l) {
-                                const float w = f1 * sf_F2(A, (float)l);
 #pragma unroll
-                                for (int bb = 0; bb < NB; ++bb) {
-                                    float *c2 = tc + (bb * TL + (l - l0)) * TK;
-                                    *c2 = fmaf(w, xv[bb], *c2);
+                            for (int j = 0; j < FLM; ++j) f2[j] = sf_F2(A, (float)(l_lo + lb + j));
+                            if (Lmax > lb + FLM) {
+#pragma unroll
+                                for (int j = FLM; j < 2 * FLM; ++j) f2[j] = sf_F2(A, (float)(l_lo + lb + j));
+                            }
+                        }
+                        float xi = xi0, g0 = sf_G(T, xi0);
+                        float *cp0 = base + lb * FTK;
+                        for (int jk = 0; jk < Kmax; ++jk) {
+                            if (jk >= j_a && jk <= jb) {
+                                xi += 1.0f;
+                                const float g1 = sf_G(T, xi);
+                                const float f1 = g1 - g0;
+                                g0 = g1;
+                                float *cpt = cp0 + jk;
+                                if (DIM == 3) {
+                                    const float w = f1 * xv[0];
+                                    if (lb == 0) {
+                                        // rows past l_hi carry weight 0 or fall into the pad rows
+#pragma unroll
+                                        for (int j = 0; j < FLM; ++j) cpt[j * FTK] = fmaf(w, f2[j], cpt[j * FTK]);
+                                    } else {
+#pragma unroll
+                                        for (int j = 0; j < FLM; ++j)
+                                            if (lb + j < L) cpt[j * FTK] = fmaf(w, f2[j], cpt[j * FTK]);
+                                    }
+                                    if (Lmax > lb + FLM) {
+#pragma unroll
+                                        for (int j = FLM; j < 2 * FLM; ++j)
+                                            if (lb + j < L) cpt[j * FTK] = fmaf(w, f2[j], cpt[j * FTK]);
+                                    }
+                                } else {
+#pragma unroll
+                                    for (int bb = 0; bb < NB; ++bb) cpt[bb * FTK] = fmaf(f1, xv[bb], cpt[bb * FTK]);
                                 }
                             }
-                        } else {
-#pragma unroll
-                            for (int bb = 0; bb < NB; ++bb) {
-                                float *c2 = tc + bb * TL * TK;
-                                *c2 = fmaf(f1, xv[bb], *c2);
-                            }
+                            __syncwarp();
                         }
                     }
                 }
-                __syncthreads();
             }
         }
     }
-    __syncthreads();
+    __syncwarp();
     // every cell of the tile is stored exactly once
-    for (int i = tid; i < NB * tlh * tkw; i += FP_THREADS) {
-        const int k = i % tkw, r = i / tkw, l = r % tlh, bb = r / tlh;
-        proj[(size_t)(b0 + bb) * proj_bstride + ((size_t)jview * pr.nv + (l0 + l)) * pr.nu + (k0 + k)] =
-            tile[(bb * TL + l) * TK + k];
+    if (DIM == 3) {
+        float *o = proj + (size_t)b0 * proj_bstride + ((size_t)jview * pr.nv + l0) * pr.nu + k0;
+        for (int l = 0; l < tlh; ++l)
+            for (int k = lane; k < tkw; k += 32) o[(size_t)l * pr.nu + k] = tile[l * FTK + k];
+    } else {
+#pragma unroll
+        for (int bb = 0; bb < NB; ++bb) {
+            float *o = proj + (size_t)(b0 + bb) * proj_bstride + (size_t)jview * pr.nu + k0;
+            for (int k = lane; k < tkw; k += 32) o[k] = tile[bb * FTK + k];
+        }
     }
 }
 
@@ -191,16 +292,17 @@ void launch_fp(const ct_geom *g, const float *d_vol, const float *d_volT, float 
                int vb, int vs, int vc, cudaStream_t st)
 {
     const SfProblem &pr = g->prob;
-    const int TK = DIM == 3 ? 128 : 256, TL = DIM == 3 ? (pr.nv >= 64 ? 64 : (pr.nv >= 32 ? 32 : 16)) : 1;
-    const int tiles_k = (pr.nu + TK - 1) / TK, tiles_l = (pr.nv + TL - 1) / TL;
+    const int tiles_k = (pr.nu + FTK - 1) / FTK, bands_l = DIM == 3 ? (pr.nv + FTL - 1) / FTL : 1;
     const size_t vbs = (size_t)pr.nx * pr.ny * pr.nz, pbs = (size_t)vc * pr.nv * pr.nu;
-    const size_t smem = (size_t)NB * TK * TL * sizeof(float);
-    auto kern = fp_tile_kernel<DIM, ARC, NB>;
+    constexpr int ROWS = DIM == 3 ? FTL + FLM : NB;
+    const size_t smem = (size_t)FPW * ROWS * FTK * sizeof(float);
+    auto kern = fp_band_kernel<DIM, ARC, NB>;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    dim3 grid(tiles_k * tiles_l, vc, groups);
-    kern<<<grid, FP_THREADS, smem, st>>>(pr, g->d_fp, d_vol + (size_t)b0 * vbs,
-                                         d_volT ? d_volT + (size_t)b0 * vbs : nullptr,
-                                         d_proj + (size_t)b0 * pbs, vb, vs, TK, TL, tiles_k, vbs, pbs);
+    const long n_items = (long)tiles_k * bands_l * vc;
+    dim3 grid((unsigned)((n_items + FPW - 1) / FPW), groups, 1);
+    kern<<<grid, 32 * FPW, smem, st>>>(pr, g->d_fp, d_vol + (size_t)b0 * vbs,
+                                       d_volT ? d_volT + (size_t)b0 * vbs : nullptr,
+                                       d_proj + (size_t)b0 * pbs, vb, vs, tiles_k, bands_l, (int)n_items, vbs, pbs);
 }
 
 template <int DIM, int ARC>

@@ -26,7 +26,7 @@ struct SfView {
     float haz, hbz, hcz;
     int32_t untilted;          // 1: az == bz == 0 and cp == cq == 0 (transaxial part independent of z)
     int32_t swap_xy;           // forward only: 1 when (p, q) = (iy, ix)
-    // ---- forward projector only: tile -> voxel-region inverse map and colouring ------------------
+    // ---- forward projector only: tile -> voxel-region inverse map -------------------------------
     // ray through detector point (kf, lf), in index space: dir = Dm + (kf - ku0c)*U + (lf - lv0c)*V (flat)
     // arc: dir = sin(g)*U + cos(g)*Dm + (lf - lv0c)*V with g = (kf - ku0c)/Ru   (U, Dm scaled by R)
     float Sp, Sq, Sz;          // source in index space
@@ -35,8 +35,8 @@ struct SfView {
     float Vp, Vq, Vz;
     float ku0c, lv0c;          // detector coordinates (cells) of the point the Dm ray hits
     float ek, el;              // tile expansion (cells / rows): max |footprint half extent| + margin
-    int32_t col_p, col_z;      // colouring strides: same-colour voxels of a slab have disjoint footprints
-    int32_t pad0, pad1;
+    int32_t lane_stride;       // voxels p, p + lane_stride project >= 1 cell apart (conflict-free rounds)
+    int32_t pad0, pad1, pad2;
 };
 
 struct SfProblem {
