@@ -71,7 +71,7 @@ constexpr int FLM = 4;            // pad rows: the first FLM footprint rows are 
 constexpr unsigned FULL = 0xffffffffu;
 
 template <int DIM, int ARC, int NB>
-__global__ void __launch_bounds__(32 * FPW)
+__global__ void __launch_bounds__(32 * FPW, 3)
 fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ vol,
                const float *__restrict__ volT, float *__restrict__ proj, int view_begin, int view_stride,
                int tiles_k, int bands_l, int n_items, size_t vol_bstride, size_t proj_bstride)
@@ -110,6 +110,7 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
     const float *src = (v.swap_xy ? volT : vol) + (size_t)b0 * vol_bstride;
     const int sp = max(1, v.lane_stride);
     const int k_top = k0 + tkw - 1, l_top = l0 + tlh - 1;
+    const int zstride = np * nq;
 
     for (int iq = 0; iq < nq; ++iq) {
         // ---- voxel region of this slab that can touch the tile (warp-uniform) --------------------
@@ -164,8 +165,9 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
             const int rs = multi ? max(nprc, 16) : max(nprc, 32);
             const int total = DIM == 3 ? nrows * rs : nprc;
             const int H = (nrows + 1) >> 1;
-            int row = 0, pi = lane;
-            while (pi >= rs) { pi -= rs; ++row; }
+            int row = 0, pi = lane;                      // rs >= 16: a step of 32 wraps at most twice
+            if (pi >= rs) { pi -= rs; ++row; }
+            if (pi >= rs) { pi -= rs; ++row; }
             for (int f0 = 0; f0 < total; f0 += 32) {
                 const int ipr = p_lo + col + sp * pi;
                 const int sh = DIM == 3 ? __float2int_rn(sigma * (float)(ipr - p_lo)) : 0;
@@ -175,10 +177,11 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
                 const int ip = act ? ipr : p_lo, iz = act ? izr : 0;
                 // advance to the next pass
                 pi += 32;
-                while (pi >= rs) { pi -= rs; ++row; }
+                if (pi >= rs) { pi -= rs; ++row; }
+                if (pi >= rs) { pi -= rs; ++row; }
                 const float p = (float)ip, z = (float)iz;
                 float xv[NB];
-                const float *xp = slab + (size_t)iz * np * nq + ip;
+                const float *xp = slab + (unsigned)(iz * zstride + ip);      // < 2^31 voxels per image
 #pragma unroll
                 for (int bb = 0; bb < NB; ++bb) xv[bb] = __ldg(xp + bb * vol_bstride);
                 const float a = fmaf(p, v.ap, fmaf(z, v.az, aq0)), b = fmaf(p, v.bp, fmaf(z, v.bz, bq0));
