@@ -301,15 +301,28 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
                         __syncthreads();
                     }
                     if (col_in) {
+                        // untilted frames: the transaxial footprint does not depend on z -> once per column
+                        const bool unt = v.untilted != 0;
+                        float a = a_col, b = b_col, inv_a = 0.0f;
+                        SfTrans T;
+                        int k_lo = 0, k_hi = -1;
+                        if (unt) {
+                            inv_a = rcp_nr(a);
+                            sf_transaxial<ARC>(v, a, b, inv_a, T);
+                            k_lo = max(max(0, tk0), (int)floorf(T.kc + T.t0));
+                            k_hi = min(min(pr.nu - 1, tk0 + TW - 1), (int)floorf(T.kc + T.t3));
+                        }
                         for (int zi = 0; zi <= z1 - z0; ++zi) {
                             const float z = (float)(z0 + zi);
-                            const float a = fmaf(z, v.az, a_col), b = fmaf(z, v.bz, b_col), c = fmaf(z, v.cz, c_col);
-                            const float inv_a = rcp_nr(a);
-                            SfTrans T;
-                            sf_transaxial<ARC>(v, a, b, inv_a, T);
-                            const int k_lo = max(max(0, tk0), (int)floorf(T.kc + T.t0));
-                            const int k_hi = min(min(pr.nu - 1, tk0 + TW - 1), (int)floorf(T.kc + T.t3));
+                            if (!unt) {
+                                a = fmaf(z, v.az, a_col); b = fmaf(z, v.bz, b_col);
+                                inv_a = rcp_nr(a);
+                                sf_transaxial<ARC>(v, a, b, inv_a, T);
+                                k_lo = max(max(0, tk0), (int)floorf(T.kc + T.t0));
+                                k_hi = min(min(pr.nu - 1, tk0 + TW - 1), (int)floorf(T.kc + T.t3));
+                            }
                             if (k_lo > k_hi) continue;
+                            const float c = fmaf(z, v.cz, c_col);
                             SfAxial A;
                             sf_axial<ARC>(v, a, b, c, inv_a, A);
                             const int l_lo = max(max(0, tl0), (int)floorf(A.lc + A.tlo));
