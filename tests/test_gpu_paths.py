@@ -1,0 +1,95 @@
+"""GPU parity on the kernels' special code paths (each case names the path it forces):
+footprints much larger / much smaller than a detector cell, arc detector in a tilted frame (reading R8),
+off-centre anisotropic volumes, regions too small for multi-row passes, view-specific magnification.
+Same tolerances as test_gpu_parity.py (BASELINE.json north_star)."""
+import math
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle.sf_oracle import Oracle
+from paper_2503_16741_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def _check(gpu, ref, what, rel_tol=1e-5, max_tol=1e-4):
+    gpu = gpu.double().cpu().numpy()
+    rel = np.linalg.norm(gpu - ref) / np.linalg.norm(ref)
+    mx = np.abs(gpu - ref).max() / np.abs(ref).max()
+    assert rel <= rel_tol and mx <= max_tol, "%s: rel-L2 %.3e max-abs/max %.3e" % (what, rel, mx)
+
+
+def _pair(c, what, seed=0):
+    """A and A^T against the oracle plus the GPU adjoint identity, for config dict c."""
+    from paper_2503_16741_b200.projector import Geometry
+    g = W.geom_keys(c)
+    x = W.make_phantom(c)
+    o, geom = Oracle(g), Geometry(g)
+    y_ref = o.fp(x)
+    y = geom.fp(torch.from_numpy(x).cuda())
+    _check(y, y_ref, "A " + what)
+    y32 = y_ref.astype(np.float32)
+    _check(geom.bp(torch.from_numpy(y32).cuda()), o.bp(y32), "A^T " + what)
+    rng = np.random.default_rng(seed)
+    xr = torch.from_numpy(rng.uniform(0, 1, x.shape).astype(np.float32)).cuda()
+    yr = torch.from_numpy(rng.uniform(0, 1, y_ref.shape).astype(np.float32)).cuda()
+    lhs = torch.sum(geom.fp(xr).double() * yr.double()).item()
+    rhs = torch.sum(xr.double() * geom.bp(yr).double()).item()
+    assert abs(lhs - rhs) <= 1e-5 * abs(lhs), (what, lhs, rhs)
+    geom.close()
+
+
+def test_large_footprints():
+    """Cells 8x smaller than a voxel's shadow: K, L ~ 20 (FP: more than 8 footprint rows -> row-chunk loop;
+    BP: several row chunks per voxel, shadows larger than one TMA box)."""
+    c = W.make_config(2, nx=24, ny=22, nz=20, nu=320, nv=300, n_views=7)
+    _pair(c, "large footprints (3-D flat)")
+    c = W.make_config(1, nx=30, ny=28, nu=500, n_views=9)
+    _pair(c, "large footprints (2-D flat)")
+
+
+def test_small_footprints_lane_stride():
+    """Cells 4x larger than a voxel's shadow: neighbouring voxels fall into the same cell, so the forward
+    kernel must use a lane stride > 1 (and its run-time conflict check must hold)."""
+    c = W.make_config(2, nx=96, ny=90, nz=40, nu=40, nv=36, n_views=9)
+    _pair(c, "small footprints (3-D flat)")
+    c = W.make_config(5, nx=200, ny=190, nu=60, n_views=11, batch=3)
+    _pair(c, "small footprints (2-D arc, batch 3)")
+    c = W.make_config(3, nx=120, ny=110, nz=24, nu=90, nv=16, n_views=9)
+    _pair(c, "small footprints (3-D arc)")
+
+
+def test_arc_detector_in_tilted_frame():
+    """Reading R8: arc detector with view-specific tilt and in-plane rotation (no BASELINE config has it)."""
+    c = W.make_config(3, nx=48, ny=44, nz=30, nu=150, nv=40, n_views=8)
+    n = c["n_views"]
+    theta = 2.0 * math.pi * np.arange(n) / n
+    phi = np.radians(12.0) * np.sin(2.0 * theta + 0.3)
+    psi = np.radians(0.4) * np.cos(theta)
+    src, dc, u, v = W.trajectory(n, c["sad"], c["sdd"], c["det_type"], theta, phi, psi)
+    c.update(src=src, det_center=dc, det_u=u, det_v=v)
+    _pair(c, "arc, tilted")
+
+
+def test_offcentre_anisotropic_volume():
+    c = W.make_config(4, nx=40, ny=52, nz=28, nu=120, nv=96, n_views=9)
+    c["dx"] *= 1.3
+    c["dz"] *= 0.6
+    c["ox"], c["oy"], c["oz"] = 7.5, -11.0, 4.0
+    _pair(c, "off-centre anisotropic (3-D flat, jittered)")
+    c = W.make_config(1, nx=50, ny=36, nu=200, n_views=10)
+    c["dy"] *= 1.7
+    c["ox"], c["oy"] = -9.0, 6.0
+    _pair(c, "off-centre anisotropic (2-D flat)")
+
+
+def test_thin_volumes_and_detectors():
+    """Few slices / few rows: the forward sweep has too few region rows for multi-row passes; the
+    backprojector's brick is mostly empty in z."""
+    c = W.make_config(2, nx=64, ny=60, nz=3, nu=150, nv=5, n_views=7)
+    _pair(c, "3 slices, 5 rows")
+    c = W.make_config(3, nx=70, ny=66, nz=2, nu=160, nv=3, n_views=6)
+    _pair(c, "2 slices, 3 rows (arc)")
