@@ -74,7 +74,7 @@ template <int DIM, int ARC, int NB>
 __global__ void __launch_bounds__(32 * FPW, 3)
 fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ vol,
                const float *__restrict__ volT, float *__restrict__ proj, int view_begin, int view_stride,
-               int tiles_k, int bands_l, int n_items, size_t vol_bstride, size_t proj_bstride)
+               int tiles_k, int bands_l, int n_items, int n_views_sel, size_t vol_bstride, size_t proj_bstride)
 {
     constexpr int ROWS = DIM == 3 ? FTL + FLM : NB;
     extern __shared__ float smem[];
@@ -83,8 +83,13 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int item = blockIdx.x * FPW + warp;
     if (item >= n_items) return;                     // warps are independent: no block barrier below
+    // item order: groups of FPW consecutive views; within a group tile-major, view fastest -- the
+    // warps of one CTA sweep the SAME tile of FPW neighbouring views, whose frusta nearly coincide,
+    // so the volume is pulled through L1/L2 once per group of views instead of once per view
     const int per_view = tiles_k * bands_l;
-    const int jview = item / per_view, rem = item - jview * per_view;
+    const int grp = item / (per_view * FPW), rem_g = item - grp * (per_view * FPW);
+    const int rem = rem_g / FPW, jview = grp * FPW + (rem_g - rem * FPW);
+    if (jview >= n_views_sel) return;
     const int bl = rem / tiles_k, tk = rem - bl * tiles_k;
     const int k0 = tk * FTK, l0 = bl * FTL;
     const int tkw = min(FTK, pr.nu - k0), tlh = DIM == 3 ? min(FTL, pr.nv - l0) : 1;
@@ -301,11 +306,11 @@ void launch_fp(const ct_geom *g, const float *d_vol, const float *d_volT, float 
     const size_t smem = (size_t)FPW * ROWS * FTK * sizeof(float);
     auto kern = fp_band_kernel<DIM, ARC, NB>;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    const long n_items = (long)tiles_k * bands_l * vc;
+    const long n_items = (long)tiles_k * bands_l * ((vc + FPW - 1) / FPW) * FPW;
     dim3 grid((unsigned)((n_items + FPW - 1) / FPW), groups, 1);
     kern<<<grid, 32 * FPW, smem, st>>>(pr, g->d_fp, d_vol + (size_t)b0 * vbs,
                                        d_volT ? d_volT + (size_t)b0 * vbs : nullptr,
-                                       d_proj + (size_t)b0 * pbs, vb, vs, tiles_k, bands_l, (int)n_items, vbs, pbs);
+                                       d_proj + (size_t)b0 * pbs, vb, vs, tiles_k, bands_l, (int)n_items, vc, vbs, pbs);
 }
 
 template <int DIM, int ARC>
