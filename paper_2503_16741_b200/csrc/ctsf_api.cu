@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <mutex>
 #include <new>
 
 #include "ctsf_internal.h"
@@ -10,6 +11,30 @@
 namespace {
 
 bool finite_pos(double x) { return std::isfinite(x) && x > 0.0; }
+
+constexpr int MAX_DEV = 64;
+cudaMemPool_t g_pool[MAX_DEV];
+std::mutex g_pool_mu;
+
+cudaMemPool_t pool_of_current_device()
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEV) { cudaGetLastError(); return nullptr; }
+    std::lock_guard<std::mutex> lock(g_pool_mu);
+    if (!g_pool[dev]) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool = nullptr;
+        if (cudaMemPoolCreate(&pool, &props) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        unsigned long long keep = ~0ull;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        g_pool[dev] = pool;
+    }
+    return g_pool[dev];
+}
 
 ct_status_t check_call(const ct_geom *g, const void *a, const void *b, int batch, int vb, int vs, int vc)
 {
@@ -21,6 +46,21 @@ ct_status_t check_call(const ct_geom *g, const void *a, const void *b, int batch
 }
 
 }  // namespace
+
+void *ctsf_alloc_async(size_t bytes, void *stream)
+{
+    void *p = nullptr;
+    cudaMemPool_t pool = pool_of_current_device();
+    cudaError_t e = pool ? cudaMallocFromPoolAsync(&p, bytes, pool, (cudaStream_t)stream)
+                         : cudaMallocAsync(&p, bytes, (cudaStream_t)stream);
+    if (e != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return p;
+}
+
+void ctsf_free_async(void *p, void *stream)
+{
+    if (p) cudaFreeAsync(p, (cudaStream_t)stream);
+}
 
 extern "C" {
 
@@ -79,6 +119,13 @@ ct_status_t ct_geom_destroy(ct_geom_t *g)
     if (g->d_bp) cudaFree(g->d_bp);
     if (g->d_fp) cudaFree(g->d_fp);
     delete g;
+    {
+        int dev = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < MAX_DEV) {
+            std::lock_guard<std::mutex> lock(g_pool_mu);
+            if (g_pool[dev]) cudaMemPoolTrimTo(g_pool[dev], 0);      // hand cached scratch back
+        }
+    }
     return CT_OK;
 }
 
@@ -116,25 +163,82 @@ ct_status_t ct_bp_sf(const ct_geom_t *g, const float *d_proj, float *d_vol, int3
     return ct_bp_sf_views(g, d_proj, d_vol, batch, 0, 1, g->prob.n_views, stream);
 }
 
+// Host-buffer operators.  3-D, batch 1: the views are cut into chunks and the host<->device copy of
+// one chunk overlaps the kernel of its neighbour on a second stream (A: the projections of chunk c
+// go home while chunk c+1 is computed; A^T: chunk c+1 arrives while chunk c is backprojected into the
+// volume, every chunk after the first adding to it).  Other shapes: copy in, run, copy out.
 static ct_status_t host_op(const ct_geom_t *g, const float *h_in, float *h_out, int32_t batch, ct_stream_t stream, bool fwd)
 {
     if (!g || !h_in || !h_out || batch < 1) return CT_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     const SfProblem &pr = g->prob;
-    const size_t nvol = (size_t)batch * pr.nx * pr.ny * pr.nz, nproj = (size_t)batch * pr.n_views * pr.nv * pr.nu;
-    const size_t n_in = fwd ? nvol : nproj, n_out = fwd ? nproj : nvol;
-    float *d_in = nullptr, *d_out = nullptr;
-    if (cudaMallocAsync((void **)&d_in, n_in * sizeof(float), st) != cudaSuccess) { cudaGetLastError(); return CT_ERR_ALLOC; }
-    if (cudaMallocAsync((void **)&d_out, n_out * sizeof(float), st) != cudaSuccess) {
-        cudaGetLastError(); cudaFreeAsync(d_in, st); return CT_ERR_ALLOC;
-    }
+    const size_t cells = (size_t)pr.nv * pr.nu;
+    const size_t nvol = (size_t)batch * pr.nx * pr.ny * pr.nz, nproj = (size_t)batch * pr.n_views * cells;
+    float *d_vol = nullptr, *d_proj = nullptr;
+    d_vol = (float *)ctsf_alloc_async(nvol * sizeof(float), st);
+    if (!d_vol) return CT_ERR_ALLOC;
+    d_proj = (float *)ctsf_alloc_async(nproj * sizeof(float), st);
+    if (!d_proj) { ctsf_free_async(d_vol, st); return CT_ERR_ALLOC; }
     ct_status_t rc = CT_OK;
-    if (cudaMemcpyAsync(d_in, h_in, n_in * sizeof(float), cudaMemcpyHostToDevice, st) != cudaSuccess) rc = CT_ERR_CUDA;
-    if (rc == CT_OK) rc = fwd ? ct_fp_sf(g, d_in, d_out, batch, stream) : ct_bp_sf(g, d_in, d_out, batch, stream);
-    if (rc == CT_OK && cudaMemcpyAsync(h_out, d_out, n_out * sizeof(float), cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = CT_ERR_CUDA;
-    cudaFreeAsync(d_in, st);
-    cudaFreeAsync(d_out, st);
+    int launches = 0;
+    const int n_chunks = (pr.dim == 3 && batch == 1) ? (pr.n_views >= 64 ? 8 : (pr.n_views >= 8 ? 2 : 1)) : 1;
+    if (n_chunks == 1) {
+        const float *d_in = fwd ? d_vol : d_proj;
+        float *d_out = fwd ? d_proj : d_vol;
+        const size_t n_in = fwd ? nvol : nproj, n_out = fwd ? nproj : nvol;
+        if (cudaMemcpyAsync((void *)d_in, h_in, n_in * sizeof(float), cudaMemcpyHostToDevice, st) != cudaSuccess) rc = CT_ERR_CUDA;
+        if (rc == CT_OK) rc = fwd ? ct_fp_sf(g, d_in, d_out, batch, stream) : ct_bp_sf(g, d_in, d_out, batch, stream);
+        launches = g->last_launches.load();
+        if (rc == CT_OK && cudaMemcpyAsync(h_out, d_out, n_out * sizeof(float), cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = CT_ERR_CUDA;
+    } else {
+        cudaStream_t cs = nullptr;                      // copy stream
+        cudaEvent_t ev[8] = {}, start = nullptr;
+        if (cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking) != cudaSuccess) rc = CT_ERR_CUDA;
+        if (rc == CT_OK && cudaEventCreateWithFlags(&start, cudaEventDisableTiming) != cudaSuccess) rc = CT_ERR_CUDA;
+        for (int c = 0; c < n_chunks && rc == CT_OK; ++c)
+            if (cudaEventCreateWithFlags(&ev[c], cudaEventDisableTiming) != cudaSuccess) rc = CT_ERR_CUDA;
+        if (rc == CT_OK) {
+            // the copy stream may not touch the buffers before `st` has reached this call (allocation order)
+            cudaEventRecord(start, st);
+            cudaStreamWaitEvent(cs, start, 0);
+            if (fwd && cudaMemcpyAsync(d_vol, h_in, nvol * sizeof(float), cudaMemcpyHostToDevice, st) != cudaSuccess) rc = CT_ERR_CUDA;
+        }
+        for (int c = 0; c < n_chunks && rc == CT_OK; ++c) {
+            const int v0 = (int)((long)pr.n_views * c / n_chunks), v1 = (int)((long)pr.n_views * (c + 1) / n_chunks);
+            const size_t off = (size_t)v0 * cells, cnt = (size_t)(v1 - v0) * cells;
+            if (fwd) {
+                rc = ct_fp_sf_views(g, d_vol, d_proj + off, 1, v0, 1, v1 - v0, stream);
+                launches += g->last_launches.load();
+                cudaEventRecord(ev[c], st);
+                cudaStreamWaitEvent(cs, ev[c], 0);
+                if (rc == CT_OK && cudaMemcpyAsync(h_out + off, d_proj + off, cnt * sizeof(float), cudaMemcpyDeviceToHost, cs) != cudaSuccess) rc = CT_ERR_CUDA;
+            } else {
+                if (cudaMemcpyAsync(d_proj + off, h_in + off, cnt * sizeof(float), cudaMemcpyHostToDevice, cs) != cudaSuccess) rc = CT_ERR_CUDA;
+                cudaEventRecord(ev[c], cs);
+                cudaStreamWaitEvent(st, ev[c], 0);
+                if (rc == CT_OK) {
+                    const int n = ctsf_launch_bp(g, d_proj + off, d_vol, 1, v0, 1, v1 - v0, stream, c > 0);
+                    if (n < 0) rc = CT_ERR_CUDA; else launches += n;
+                }
+            }
+        }
+        if (!fwd && rc == CT_OK && cudaMemcpyAsync(h_out, d_vol, nvol * sizeof(float), cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = CT_ERR_CUDA;
+        if (cs) {
+            // `st` must outlive the copies of `cs` before the buffers are freed on it
+            if (start) { cudaEventRecord(start, cs); cudaStreamWaitEvent(st, start, 0); }
+        }
+        cudaFreeAsync(d_vol, st);
+        cudaFreeAsync(d_proj, st);
+        d_vol = d_proj = nullptr;
+        if (cudaStreamSynchronize(st) != cudaSuccess && rc == CT_OK) rc = CT_ERR_CUDA;
+        for (int c = 0; c < n_chunks; ++c) if (ev[c]) cudaEventDestroy(ev[c]);
+        if (start) cudaEventDestroy(start);
+        if (cs) cudaStreamDestroy(cs);
+    }
+    if (d_vol) cudaFreeAsync(d_vol, st);
+    if (d_proj) cudaFreeAsync(d_proj, st);
     if (cudaStreamSynchronize(st) != cudaSuccess && rc == CT_OK) rc = CT_ERR_CUDA;
+    const_cast<ct_geom *>(g)->last_launches.store(launches);
     if (rc != CT_OK) cudaGetLastError();
     return rc;
 }

@@ -215,7 +215,7 @@ template <int ARC>
 __global__ void __launch_bounds__(BRICK_THREADS, 3)
 bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ proj,
                 const __grid_constant__ CUtensorMap tmap, int use_tma, float *__restrict__ vol,
-                int view_begin, int view_stride, int view_count, int nbz)
+                int view_begin, int view_stride, int view_count, int j_lo, int j_hi, int nbz, int accumulate)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float *tile0 = reinterpret_cast<float *>(smem_raw);
@@ -276,12 +276,12 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
     };
 
     uint32_t phase[2] = {0u, 0u};
-    if (warp == 0 && view_count > 0) prefetch(0, 0);
+    if (warp == 0 && j_lo < j_hi) prefetch(j_lo, j_lo & 1);
     __syncthreads();
 
-    for (int j = 0; j < view_count; ++j) {
+    for (int j = j_lo; j < j_hi; ++j) {         // this launch's chunk of the call's views
         const int s = j & 1;
-        if (warp == 0 && j + 1 < view_count) prefetch(j + 1, s ^ 1);
+        if (warp == 0 && j + 1 < j_hi) prefetch(j + 1, s ^ 1);
         const TileInfo t = tinfo[s];
         if (t.live) {
             const SfView &v = sview[s];
@@ -340,7 +340,11 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
     }
     if (col_in) {
         float *o = vol + (size_t)batch * pr.nx * pr.ny * pr.nz + ((size_t)z0 * pr.ny + iq) * pr.nx + ip;
-        for (int zi = 0; zi <= z1 - z0; ++zi) o[(size_t)zi * pr.ny * pr.nx] = accs[zi * BRICK_THREADS + tid];
+        for (int zi = 0; zi <= z1 - z0; ++zi) {
+            float *oz = o + (size_t)zi * pr.ny * pr.nx;
+            const float r = accs[zi * BRICK_THREADS + tid];
+            *oz = accumulate ? *oz + r : r;          // accumulate: view-chunked host pipeline only
+        }
     }
 }
 
@@ -366,7 +370,8 @@ EncodeTiledFn get_encode()
 }
 
 template <int ARC>
-int launch_brick(const ct_geom *g, const float *d_proj, float *d_vol, int batch, int vb, int vs, int vc, cudaStream_t st)
+int launch_brick(const ct_geom *g, const float *d_proj, float *d_vol, int batch, int vb, int vs, int vc, cudaStream_t st,
+                 int accumulate)
 {
     const SfProblem &pr = g->prob;
     CUtensorMap tmap;
@@ -388,15 +393,28 @@ int launch_brick(const ct_geom *g, const float *d_proj, float *d_vol, int batch,
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const int nbz = (pr.nz + BZ - 1) / BZ;
     int launches = 0;
-    for (int b0 = 0; b0 < batch;) {
-        int nb = batch - b0;
-        if ((long)nb * nbz > 65535) nb = 65535 / nbz > 0 ? 65535 / nbz : 1;
-        dim3 grid((pr.nx + BX - 1) / BX, (pr.ny + BY - 1) / BY, nbz * nb);
-        // the tensor map addresses view (batch*vc + j): pass the buffer of image b0 by offsetting batch in-kernel
-        kern<<<grid, BRICK_THREADS, smem, st>>>(pr, g->d_bp, d_proj + (size_t)b0 * vc * pr.nv * pr.nu, tmap, b0 == 0 ? use_tma : 0,
-                                                d_vol + (size_t)b0 * pr.nx * pr.ny * pr.nz, vb, vs, vc, nbz);
-        ++launches;
-        b0 += nb;
+    // The view loop is cut into chunks of ~96 MB of projections, one launch each (every launch after the
+    // first adds to the volume): all bricks sweep one chunk while it sits in the 126 MB L2, instead of
+    // each wave of CTAs streaming the whole projection set from HBM again.
+    const size_t view_bytes = (size_t)pr.nu * pr.nv * sizeof(float) * batch;
+    int chunk = (int)((96u << 20) / (view_bytes ? view_bytes : 1));
+    if (chunk < 8) chunk = 8;
+    const char *cdbg = getenv("CTSF_BP_CHUNK");
+    if (cdbg && atoi(cdbg) > 0) chunk = atoi(cdbg);
+    for (int j_lo = 0; j_lo < vc || (vc == 0 && j_lo == 0); j_lo += chunk) {
+        const int j_hi = j_lo + chunk < vc ? j_lo + chunk : vc;
+        for (int b0 = 0; b0 < batch;) {
+            int nb = batch - b0;
+            if ((long)nb * nbz > 65535) nb = 65535 / nbz > 0 ? 65535 / nbz : 1;
+            dim3 grid((pr.nx + BX - 1) / BX, (pr.ny + BY - 1) / BY, nbz * nb);
+            // the tensor map addresses view (batch*vc + j): pass the buffer of image b0 by offsetting batch in-kernel
+            kern<<<grid, BRICK_THREADS, smem, st>>>(pr, g->d_bp, d_proj + (size_t)b0 * vc * pr.nv * pr.nu, tmap, b0 == 0 ? use_tma : 0,
+                                                    d_vol + (size_t)b0 * pr.nx * pr.ny * pr.nz, vb, vs, vc, j_lo, j_hi, nbz,
+                                                    accumulate || j_lo > 0);
+            ++launches;
+            b0 += nb;
+        }
+        if (vc == 0) break;
     }
     return launches;
 }
@@ -443,14 +461,15 @@ int launch_pixel_batches(const ct_geom *g, const float *d_proj, float *d_vol, in
 }  // namespace
 
 int ctsf_launch_bp(const ct_geom *g, const float *d_proj, float *d_vol, int batch,
-                   int view_begin, int view_stride, int view_count, void *stream)
+                   int view_begin, int view_stride, int view_count, void *stream, int accumulate)
 {
     cudaStream_t st = (cudaStream_t)stream;
     const int arc = g->prob.det_type, dim = g->prob.dim;
+    if (accumulate && dim != 3) return -1;       // only the 3-D brick kernel can add to its output
     int n;
     if (dim == 2) n = arc ? launch_pixel_batches<1>(g, d_proj, d_vol, batch, view_begin, view_stride, view_count, st)
                           : launch_pixel_batches<0>(g, d_proj, d_vol, batch, view_begin, view_stride, view_count, st);
-    else          n = arc ? launch_brick<1>(g, d_proj, d_vol, batch, view_begin, view_stride, view_count, st)
-                          : launch_brick<0>(g, d_proj, d_vol, batch, view_begin, view_stride, view_count, st);
+    else          n = arc ? launch_brick<1>(g, d_proj, d_vol, batch, view_begin, view_stride, view_count, st, accumulate)
+                          : launch_brick<0>(g, d_proj, d_vol, batch, view_begin, view_stride, view_count, st, accumulate);
     return cudaGetLastError() == cudaSuccess ? n : -1;
 }

@@ -359,7 +359,8 @@ int ctsf_launch_fp(const ct_geom *g, const float *d_vol, float *d_proj, int batc
     for (int j = 0; j < view_count && !need_T; ++j) need_T = g->h_fp[view_begin + (size_t)j * view_stride].swap_xy != 0;
     if (need_T) {
         const size_t n = (size_t)batch * pr.nx * pr.ny * pr.nz;
-        if (cudaMallocAsync((void **)&d_volT, n * sizeof(float), st) != cudaSuccess) return -1;
+        d_volT = (float *)ctsf_alloc_async(n * sizeof(float), st);
+        if (!d_volT) return -1;
         dim3 grid((pr.nx + 31) / 32, (pr.ny + 31) / 32, 1), block(32, 8);
         // one launch per chunk of <= 65535 slices
         const long slices = (long)batch * pr.nz;
@@ -375,6 +376,6 @@ int ctsf_launch_fp(const ct_geom *g, const float *d_vol, float *d_proj, int batc
                                      : launch_fp_batches<2, 0>(g, d_vol, d_volT, d_proj, batch, view_begin, view_stride, view_count, st);
     else             launches += arc ? launch_fp_batches<3, 1>(g, d_vol, d_volT, d_proj, batch, view_begin, view_stride, view_count, st)
                                      : launch_fp_batches<3, 0>(g, d_vol, d_volT, d_proj, batch, view_begin, view_stride, view_count, st);
-    if (d_volT) cudaFreeAsync(d_volT, st);
+    ctsf_free_async(d_volT, st);
     return cudaGetLastError() == cudaSuccess ? launches : -1;
 }

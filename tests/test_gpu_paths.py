@@ -93,3 +93,38 @@ def test_thin_volumes_and_detectors():
     _pair(c, "3 slices, 5 rows")
     c = W.make_config(3, nx=70, ny=66, nz=2, nu=160, nv=3, n_views=6)
     _pair(c, "2 slices, 3 rows (arc)")
+
+
+def test_host_buffer_entry_points():
+    """ct_fp_sf_host / ct_bp_sf_host (the e2e path of bench.py): view-chunked copy/compute pipeline for
+    3-D batch 1 (8 chunks at >= 64 views, A^T accumulating chunk by chunk), plain path otherwise; results
+    must equal the device-pointer operators bit for bit (A) / to rounding of the chunked sum (A^T) and
+    match the oracle within the usual tolerances."""
+    from paper_2503_16741_b200 import binding as B
+    from paper_2503_16741_b200.projector import Geometry
+    for index, shrink in ((4, dict(nx=36, ny=40, nz=30, nu=100, nv=90, n_views=67)),
+                          (2, dict(nx=30, ny=30, nz=20, nu=64, nv=60, n_views=9)),
+                          (5, dict(nx=64, ny=60, nu=150, n_views=20, batch=3))):
+        c = W.make_config(index, **shrink)
+        g = W.geom_keys(c)
+        x = W.make_phantom(c)
+        o, geom = Oracle(g), Geometry(g)
+        y_ref = o.fp(x)
+        hx = torch.from_numpy(x).pin_memory()
+        hy = torch.empty(y_ref.shape, dtype=torch.float32).pin_memory()
+        B.ct_fp_sf_host(geom.handle, hx.data_ptr(), hy.data_ptr(), c["batch"], 0)
+        assert geom.last_launch_count() > 0
+        y_dev = geom.fp(torch.from_numpy(x).cuda())
+        torch.cuda.synchronize()
+        assert torch.equal(hy, y_dev.cpu()), "A host != device, config %d" % index
+        _check(hy, y_ref, "A host config %d" % index)
+        y32 = y_ref.astype(np.float32)
+        hp = torch.from_numpy(y32).pin_memory()
+        hxb = torch.empty(x.shape, dtype=torch.float32).pin_memory()
+        B.ct_bp_sf_host(geom.handle, hp.data_ptr(), hxb.data_ptr(), c["batch"], 0)
+        _check(hxb, o.bp(y32), "A^T host config %d" % index)
+        # pageable host memory is accepted too
+        out = np.empty(y_ref.shape, np.float32)
+        B.ct_fp_sf_host(geom.handle, x.ctypes.data, out.ctypes.data, c["batch"], 0)
+        assert np.array_equal(out, hy.numpy())
+        geom.close()
