@@ -116,6 +116,7 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
     const int sp = max(1, v.lane_stride);
     const int k_top = k0 + tkw - 1, l_top = l0 + tlh - 1;
     const int zstride = np * nq;
+    const float v_ap = v.ap, v_bp = v.bp, v_cp = v.cp, v_az = v.az, v_bz = v.bz, v_cz = v.cz;
 
     for (int iq = 0; iq < nq; ++iq) {
         // ---- voxel region of this slab that can touch the tile (warp-uniform) --------------------
@@ -189,21 +190,24 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
                 const float *xp = slab + (unsigned)(iz * zstride + ip);      // < 2^31 voxels per image
 #pragma unroll
                 for (int bb = 0; bb < NB; ++bb) xv[bb] = __ldg(xp + bb * vol_bstride);
-                const float a = fmaf(p, v.ap, fmaf(z, v.az, aq0)), b = fmaf(p, v.bp, fmaf(z, v.bz, bq0));
-                const float c = DIM == 3 ? fmaf(p, v.cp, fmaf(z, v.cz, cq0)) : 0.0f;
+                const float a = fmaf(p, v_ap, fmaf(z, v_az, aq0)), b = fmaf(p, v_bp, fmaf(z, v_bz, bq0));
+                const float c = DIM == 3 ? fmaf(p, v_cp, fmaf(z, v_cz, cq0)) : 0.0f;
                 const float inv_a = rcp_nr(a);
-                SfTrans T;
-                sf_transaxial<ARC>(v, a, b, inv_a, T);
-                // unclipped column range: rounds are aligned on it, columns off the tile are skipped
-                const int k_lo = (int)floorf(T.kc + T.t0);
-                const int k_hi = (int)floorf(T.kc + T.t3);
+                // rows first: a pass whose voxels all miss the band in l (the extreme rows of the sheared
+                // region) is dropped before the costlier transaxial part
                 SfAxial A;
                 int l_lo = 0, l_hi = 0;
                 if (DIM == 3) {
                     sf_axial<ARC>(v, a, b, c, inv_a, A);
                     l_lo = max(l0, (int)floorf(A.lc + A.tlo));
                     l_hi = min(l_top, (int)floorf(A.lc + A.thi));
+                    if (!__any_sync(FULL, act && l_lo <= l_hi)) continue;
                 }
+                SfTrans T;
+                sf_transaxial<ARC>(v, a, b, inv_a, T);
+                // unclipped column range: rounds are aligned on it, columns off the tile are skipped
+                const int k_lo = (int)floorf(T.kc + T.t0);
+                const int k_hi = (int)floorf(T.kc + T.t3);
                 const bool live = act && k_hi >= k0 && k_lo <= k_top && l_lo <= l_hi;
                 // rounds j_a .. j_b of this lane update columns k_lo + j that lie on the tile
                 const int j_a = live ? max(0, k0 - k_lo) : 0;
