@@ -284,7 +284,7 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
         if (warp == 0 && j + 1 < j_hi) prefetch(j + 1, s ^ 1);
         const TileInfo t = tinfo[s];
         if (t.live) {
-            const SfView &v = sview[s];
+            const SfView v = sview[s];          // local copy: the fields in use stay in registers over the z-run
             float *tile = s ? tile1 : tile0;
             const float a_col = fmaf(q, v.aq, fmaf(p, v.ap, v.a0));
             const float b_col = fmaf(q, v.bq, fmaf(p, v.bp, v.b0));
