@@ -128,3 +128,38 @@ def test_host_buffer_entry_points():
         B.ct_fp_sf_host(geom.handle, x.ctypes.data, out.ctypes.data, c["batch"], 0)
         assert np.array_equal(out, hy.numpy())
         geom.close()
+
+
+def test_config5_gradient_descent_against_oracle():
+    """BASELINE.json config 5 (shrunken): 10 steps of x <- x - lr * 2 A^T (A x - y), y = fp32(oracle A x_true),
+    lr = 1 / (2 max_j [A^T A 1]_j) from the oracle; the GPU loop (fp32, through the C ABI) must track the
+    float64 oracle loop: every loss within 1e-4 relative, x_10 within rel-L2 1e-4 (ten operator pairs deep,
+    so ten times the single-operator budget)."""
+    from paper_2503_16741_b200.projector import Geometry
+    c = W.make_config(5, nx=72, ny=70, nu=150, n_views=30, batch=3)
+    g = W.geom_keys(c)
+    o, geom = Oracle(g), Geometry(g)
+    x_true = W.make_phantom(c, seed=c["seed"] + 100)
+    y = o.fp(x_true).astype(np.float32)
+    ones = np.ones_like(x_true)
+    lr = 1.0 / (2.0 * o.bp(o.fp(ones)).max())
+    # oracle loop, float64
+    xo = np.zeros(x_true.shape, np.float64)
+    losses_o = []
+    for _ in range(10):
+        r = o.fp(xo) - y
+        losses_o.append(float((r ** 2).sum()))
+        xo = xo - lr * 2.0 * o.bp(r)
+    # GPU loop, fp32
+    yd = torch.from_numpy(y).cuda()
+    xg = torch.zeros(x_true.shape, device="cuda")
+    losses_g = []
+    for _ in range(10):
+        r = geom.fp(xg) - yd
+        losses_g.append(float((r.double() ** 2).sum().item()))
+        xg = xg - float(lr) * 2.0 * geom.bp(r)
+    assert all(b < a for a, b in zip(losses_g, losses_g[1:])), losses_g
+    for a, b in zip(losses_g, losses_o):
+        assert abs(a - b) <= 1e-4 * abs(b), (losses_g, losses_o)
+    _check(xg, xo, "x_10 of the config-5 loop", rel_tol=1e-4, max_tol=1e-3)
+    geom.close()
