@@ -70,6 +70,33 @@ constexpr int FTL = 32;           // rows per warp tile (3-D)
 constexpr int FLM = 4;            // pad rows: the first FLM footprint rows are updated unconditionally
 constexpr unsigned FULL = 0xffffffffu;
 
+__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ float lds_f32(uint32_t a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
+__device__ __forceinline__ void sts_f32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v)); }
+
+// one round of one lane: tile[row j][its column] += w * f2[j] for the lane's rows.  FIRST: the first FLM rows are
+// updated unconditionally (weight 0 past the footprint, pad rows past the tile); EXTRA: rows FLM .. 2 FLM - 1 exist
+// for some lane of the warp.  Loads first, then FMAs, then stores (the volatile asm keeps this order).
+template <bool FIRST, bool EXTRA>
+__device__ __forceinline__ void fp_round_rows(uint32_t ca, float w, const float *f2, int nrow)
+{
+    constexpr int RB = FTK * 4;
+    if (FIRST) {
+        const float c0 = lds_f32(ca), c1 = lds_f32(ca + RB), c2 = lds_f32(ca + 2 * RB), c3 = lds_f32(ca + 3 * RB);
+        sts_f32(ca, fmaf(w, f2[0], c0)); sts_f32(ca + RB, fmaf(w, f2[1], c1));
+        sts_f32(ca + 2 * RB, fmaf(w, f2[2], c2)); sts_f32(ca + 3 * RB, fmaf(w, f2[3], c3));
+    } else {
+#pragma unroll
+        for (int j = 0; j < FLM; ++j)
+            if (j < nrow) sts_f32(ca + j * RB, fmaf(w, f2[j], lds_f32(ca + j * RB)));
+    }
+    if (EXTRA) {
+#pragma unroll
+        for (int j = FLM; j < 2 * FLM; ++j)
+            if (j < nrow) sts_f32(ca + j * RB, fmaf(w, f2[j], lds_f32(ca + j * RB)));
+    }
+}
+
 template <int DIM, int ARC, int NB>
 __global__ void __launch_bounds__(32 * FPW, 3)
 fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ vol,
@@ -248,37 +275,32 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
                             }
                         }
                         float xi = xi0, g0 = sf_G(T, xi0);
-                        float *cp0 = base + lb * FTK;
-                        for (int jk = 0; jk < Kmax; ++jk) {
-                            if (jk >= j_a && jk <= jb) {
-                                xi += 1.0f;
-                                const float g1 = sf_G(T, xi);
-                                const float f1 = g1 - g0;
-                                g0 = g1;
-                                float *cpt = cp0 + jk;
-                                if (DIM == 3) {
-                                    const float w = f1 * xv[0];
-                                    if (lb == 0) {
-                                        // rows past l_hi carry weight 0 or fall into the pad rows
-#pragma unroll
-                                        for (int j = 0; j < FLM; ++j) cpt[j * FTK] = fmaf(w, f2[j], cpt[j * FTK]);
-                                    } else {
-#pragma unroll
-                                        for (int j = 0; j < FLM; ++j)
-                                            if (lb + j < L) cpt[j * FTK] = fmaf(w, f2[j], cpt[j * FTK]);
-                                    }
-                                    if (Lmax > lb + FLM) {
-#pragma unroll
-                                        for (int j = FLM; j < 2 * FLM; ++j)
-                                            if (lb + j < L) cpt[j * FTK] = fmaf(w, f2[j], cpt[j * FTK]);
-                                    }
-                                } else {
-#pragma unroll
-                                    for (int bb = 0; bb < NB; ++bb) cpt[bb * FTK] = fmaf(f1, xv[bb], cpt[bb * FTK]);
-                                }
-                            }
-                            __syncwarp();
+                        uint32_t ca = smem_addr(base + lb * FTK);      // this lane's cell of round 0
+                        const int nrow = L - lb;
+#define CTSF_ROUNDS(...)                                             \
+                        for (int jk = 0; jk < Kmax; ++jk, ca += 4) {   \
+                            if (jk >= j_a && jk <= jb) {               \
+                                xi += 1.0f;                            \
+                                const float g1 = sf_G(T, xi);          \
+                                const float f1 = g1 - g0;              \
+                                g0 = g1;                               \
+                                __VA_ARGS__                            \
+                            }                                          \
+                            __syncwarp();                              \
                         }
+                        if (DIM == 3) {
+                            if (lb == 0 && Lmax <= FLM) {
+                                CTSF_ROUNDS(fp_round_rows<true, false>(ca, f1 * xv[0], f2, nrow);)
+                            } else if (lb == 0) {
+                                CTSF_ROUNDS(fp_round_rows<true, true>(ca, f1 * xv[0], f2, nrow);)
+                            } else {
+                                CTSF_ROUNDS(fp_round_rows<false, true>(ca, f1 * xv[0], f2, nrow);)
+                            }
+                        } else {
+                            CTSF_ROUNDS(_Pragma("unroll") for (int bb = 0; bb < NB; ++bb)
+                                            sts_f32(ca + bb * FTK * 4, fmaf(f1, xv[bb], lds_f32(ca + bb * FTK * 4)));)
+                        }
+#undef CTSF_ROUNDS
                     }
                 }
             }
