@@ -186,13 +186,8 @@ __device__ __forceinline__ float gather_tile(const float *__restrict__ tile, con
     float sum = 0.0f;
     for (int lb = l_lo; lb <= l_hi; lb += LM) {
         // rows past l_hi get weight 0 by themselves (x >= thi), rows past the tile read the zero pad rows
-        const float x0 = (float)lb - A.lc;
         float f2[LM];
-#pragma unroll
-        for (int j = 0; j < LM; ++j) {
-            const float x = x0 + (float)j;
-            f2[j] = fmaxf(fminf(x + 1.0f, A.thi) - fmaxf(x, A.tlo), 0.0f);
-        }
+        sf_F2_run<LM>(A, (float)lb, f2);
         const float *row = tile + (lb - tl0) * TW + (k_lo - tk0);
         float xi = (float)k_lo - T.kc;
         float g0 = sf_G(T, xi);

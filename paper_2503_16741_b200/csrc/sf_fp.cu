@@ -267,12 +267,8 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
                     for (int lb = 0; lb < Lmax; lb += 2 * FLM) {
                         float f2[2 * FLM];
                         if (DIM == 3) {
-#pragma unroll
-                            for (int j = 0; j < FLM; ++j) f2[j] = sf_F2(A, (float)(l_lo + lb + j));
-                            if (Lmax > lb + FLM) {
-#pragma unroll
-                                for (int j = FLM; j < 2 * FLM; ++j) f2[j] = sf_F2(A, (float)(l_lo + lb + j));
-                            }
+                            if (Lmax > lb + FLM) sf_F2_run<2 * FLM>(A, (float)(l_lo + lb), f2);
+                            else                 sf_F2_run<FLM>(A, (float)(l_lo + lb), f2);
                         }
                         float xi = xi0, g0 = sf_G(T, xi0);
                         uint32_t ca = smem_addr(base + lb * FTK);      // this lane's cell of round 0
