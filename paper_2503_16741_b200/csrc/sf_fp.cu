@@ -65,6 +65,7 @@ __device__ __forceinline__ Ray tile_ray(const SfView &v, float kf, float lf)
 // kernel verifies it with a warp match), so within a round the lanes touch pairwise different
 // columns; rounds are separated by __syncwarp().  Summation order is fixed => deterministic.
 constexpr int FPW = 8;            // warps per CTA
+constexpr int FMINB = 3;          // CTAs per SM the register budget is sized for
 constexpr int FTK = 64;           // cells per warp tile
 constexpr int FTL = 32;           // rows per warp tile (3-D)
 constexpr int FLM = 4;            // pad rows: the first FLM footprint rows are updated unconditionally
@@ -98,7 +99,7 @@ __device__ __forceinline__ void fp_round_rows(uint32_t ca, float w, const float 
 }
 
 template <int DIM, int ARC, int NB>
-__global__ void __launch_bounds__(32 * FPW, 3)
+__global__ void __launch_bounds__(32 * FPW, FMINB)
 fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ vol,
                const float *__restrict__ volT, float *__restrict__ proj, int view_begin, int view_stride,
                int tiles_k, int bands_l, int n_items, int n_views_sel, size_t vol_bstride, size_t proj_bstride)
