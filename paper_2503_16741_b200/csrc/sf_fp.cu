@@ -11,6 +11,7 @@
 #include <cuda_runtime.h>
 
 #include <climits>
+#include <cstdlib>
 
 #include "ctsf_internal.h"
 #include "sf_footprint.cuh"
@@ -102,7 +103,8 @@ template <int DIM, int ARC, int NB>
 __global__ void __launch_bounds__(32 * FPW, FMINB)
 fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ vol,
                const float *__restrict__ volT, float *__restrict__ proj, int view_begin, int view_stride,
-               int tiles_k, int bands_l, int n_items, int n_views_sel, size_t vol_bstride, size_t proj_bstride)
+               int tiles_k, int bands_l, int n_items, int n_views_sel, size_t vol_bstride, size_t proj_bstride,
+               float region_pad)
 {
     constexpr int ROWS = DIM == 3 ? FTL + FLM : NB;
     extern __shared__ float smem[];
@@ -130,13 +132,31 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
     for (int i = lane; i < ROWS * FTK; i += 32) tile[i] = 0.0f;
     __syncwarp();
     const SfView &v = sviews[warp];
+    // Rays through the tile's corners (and, for the arc, the mid column: the slab image of an arc tile
+    // bulges).  The surfaces k = const and (flat) l = const through the source are planes, so they cut a
+    // slab in straight lines and the tile's pre-image in the slab is the quadrilateral spanned by the
+    // rays.  A voxel touches the tile iff one of its four transaxial corners (+-1/2, +-1/2) / its two
+    // axial end points (0, 0, +-1/2) cross those lines, i.e. iff its centre lies within
+    // hp = 1/2 + 1/2 |dp/dq| voxels in p and 1/2 voxel in z of the quadrilateral.
+    float slope = 0.0f;
     if (lane < 6) {
-        // expanded tile: corners (and, for the arc, the mid column: the slab image of an arc tile bulges)
-        const float kA = (float)k0 - v.ek, kB = (float)(k0 + tkw) + v.ek;
-        const float lA = (float)l0 - v.el, lB = (float)(l0 + tlh) + v.el;
+        const float kA = (float)k0, kB = (float)(k0 + tkw), lA = (float)l0, lB = (float)(l0 + tlh);
         const float kk = (lane % 3 == 0) ? kA : (lane % 3 == 1 ? kB : 0.5f * (kA + kB));
-        srays[warp][lane] = tile_ray<ARC>(v, kk, lane < 3 ? lA : lB);
+        const Ray ry = tile_ray<ARC>(v, kk, lane < 3 ? lA : lB);
+        srays[warp][lane] = ry;
+        // direction of the line {k = const, z = const} in the slab plane: the ray minus its z part along v
+        float dp = ry.dp, dq = ry.dq;
+        if (DIM == 3 && fabsf(v.Vz) > 1e-6f) {
+            const float t = ry.dz / v.Vz;
+            dp = fmaf(-t, v.Vp, dp); dq = fmaf(-t, v.Vq, dq);
+        }
+        slope = fabsf(dp) / fmaxf(fabsf(dq), 1e-6f);
     }
+#pragma unroll
+    for (int s_ = 1; s_ < 8; s_ <<= 1) slope = fmaxf(slope, __shfl_xor_sync(FULL, slope, s_));
+    slope = __shfl_sync(FULL, slope, 0);
+    const float hp = 0.6f + 0.5f * fminf(slope, 4.0f) + region_pad;
+    const float hz = (ARC ? 1.5f : 1.1f) + region_pad;            // 1/2 voxel + 1/2 (rounded shear shift) + margin (arc: bulge)
     __syncwarp();
 
     const int np = v.swap_xy ? pr.ny : pr.nx, nq = v.swap_xy ? pr.nx : pr.ny, nz = pr.nz;
@@ -166,7 +186,7 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
         int p_lo = 0, p_hi = np - 1, zs_lo = 0, zs_hi = nz - 1;
         float sigma = 0.0f;
         if (!whole) {
-            p_lo = max(0, (int)ceilf(pmin - 0.3f)); p_hi = min(np - 1, (int)floorf(pmax + 0.3f));
+            p_lo = max(0, (int)ceilf(pmin - hp)); p_hi = min(np - 1, (int)floorf(pmax + hp));
             if (DIM == 3) {
                 // mean slope dz/dp of the two tile edges l = const (rays 0,1 and 3,4)
                 const float dpp = (pr_[1] - pr_[0]) + (pr_[4] - pr_[3]);
@@ -179,8 +199,8 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
                     zmin = fminf(zmin, zs); zmax = fmaxf(zmax, zs);
                 }
                 const float smax = sigma * (float)(p_hi - p_lo);           // shift range over the region
-                zs_lo = max((int)ceilf(zmin - 0.8f), -(int)ceilf(fmaxf(smax, 0.0f)) - 1);
-                zs_hi = min((int)floorf(zmax + 0.8f), nz + (int)ceilf(fmaxf(-smax, 0.0f)));
+                zs_lo = max((int)ceilf(zmin - hz), -(int)ceilf(fmaxf(smax, 0.0f)) - 1);
+                zs_hi = min((int)floorf(zmax + hz), nz + (int)ceilf(fmaxf(-smax, 0.0f)));
             }
         }
         if (p_lo > p_hi || zs_lo > zs_hi) continue;
@@ -330,10 +350,14 @@ void launch_fp(const ct_geom *g, const float *d_vol, const float *d_volT, float 
     auto kern = fp_band_kernel<DIM, ARC, NB>;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const long n_items = (long)tiles_k * bands_l * ((vc + FPW - 1) / FPW) * FPW;
+    // testing aid: CTSF_FP_PAD=<voxels> widens the swept voxel region; the result must not change beyond
+    // summation order (tests/test_gpu_fullsize.py uses it to prove that the tight region misses nothing)
+    const char *pad_env = getenv("CTSF_FP_PAD");
+    const float region_pad = pad_env ? (float)atof(pad_env) : 0.0f;
     dim3 grid((unsigned)((n_items + FPW - 1) / FPW), groups, 1);
     kern<<<grid, 32 * FPW, smem, st>>>(pr, g->d_fp, d_vol + (size_t)b0 * vbs,
                                        d_volT ? d_volT + (size_t)b0 * vbs : nullptr,
-                                       d_proj + (size_t)b0 * pbs, vb, vs, tiles_k, bands_l, (int)n_items, vc, vbs, pbs);
+                                       d_proj + (size_t)b0 * pbs, vb, vs, tiles_k, bands_l, (int)n_items, vc, vbs, pbs, region_pad);
 }
 
 template <int DIM, int ARC>

@@ -57,3 +57,29 @@ def test_parity_full_size_sampled(index):
         mx = np.abs(got - ref).max() / np.abs(ref).max()
         assert rel <= 1e-5 and mx <= 1e-4, "A^T config %d: rel-L2 %.3e max %.3e" % (index, rel, mx)
     geom.close()
+
+
+@pytest.mark.parametrize("index", [4, 3, 2])
+def test_forward_region_is_conservative(index, monkeypatch):
+    """The forward kernel sweeps, per slab, only the voxels its tile's frustum can touch (exact half-voxel halo).
+    Property that holds at any size: widening that region by a whole voxel (CTSF_FP_PAD) may only change the
+    summation order.  Checked on EVERY cell of every view of the full-size operator (a missed voxel would
+    shift a cell by ~1e-3 of its value)."""
+    from paper_2503_16741_b200.projector import Geometry
+    c = W.make_config(index)
+    if index == 4:
+        c = W.make_config(index, n_views=96)          # every 7.5th view of the trajectory, full volume/detector
+    g = W.geom_keys(c)
+    rng = np.random.default_rng(77 + index)
+    x = torch.from_numpy(rng.uniform(0.5, 1.5, (1, c["nz"], c["ny"], c["nx"])).astype(np.float32)).cuda()
+    geom = Geometry(g)
+    monkeypatch.delenv("CTSF_FP_PAD", raising=False)
+    y_tight = geom.fp(x)
+    torch.cuda.synchronize()
+    monkeypatch.setenv("CTSF_FP_PAD", "1.0")
+    y_wide = geom.fp(x)
+    torch.cuda.synchronize()
+    monkeypatch.delenv("CTSF_FP_PAD")
+    diff = (y_tight - y_wide).abs().max().item()
+    assert diff <= 3e-6 * y_wide.abs().max().item(), diff
+    geom.close()
