@@ -83,3 +83,21 @@ def test_forward_region_is_conservative(index, monkeypatch):
     diff = (y_tight - y_wide).abs().max().item()
     assert diff <= 3e-6 * y_wide.abs().max().item(), diff
     geom.close()
+
+
+@pytest.mark.parametrize("index", [2, 5])
+def test_run_to_run_determinism(index):
+    """Both operators fix their summation order (no atomics; the forward kernel's conflict-free rounds), so
+    repeated calls are bit-identical.  A shared-memory race in the forward tile would show up here."""
+    from paper_2503_16741_b200.projector import Geometry
+    c = W.make_config(index)
+    g = W.geom_keys(c)
+    rng = np.random.default_rng(5 + index)
+    x = torch.from_numpy(rng.uniform(0, 1, (c["batch"], c["nz"], c["ny"], c["nx"])).astype(np.float32)).cuda()
+    geom = Geometry(g)
+    y0 = geom.fp(x)
+    xb0 = geom.bp(y0)
+    for _ in range(2):
+        assert torch.equal(geom.fp(x), y0)
+        assert torch.equal(geom.bp(y0), xb0)
+    geom.close()
