@@ -12,6 +12,7 @@ struct ct_geom {
     SfView *d_bp = nullptr, *d_fp = nullptr;
     int any_swap = 0;                 // some forward view reads the volume through its transpose
     int all_untilted = 0;             // every view: transaxial footprint independent of z
+    int fp_hoist_ok = 0;              // all untilted AND every footprint spans <= 6 columns, <= 8 rows
     int device = 0;
     std::atomic<int> last_launches{0};
 };

@@ -41,6 +41,7 @@ ct_status_t ctsf_build_views(const ct_geom_desc_t *d, ct_geom *g)
     g->h_fp.resize(nviews);
     g->any_swap = 0;
     g->all_untilted = 1;
+    int small_fp = 1;
     // world position of voxel (0,0,0)
     const V3 O = {d->ox - 0.5 * (d->nx - 1) * d->dx, d->oy - 0.5 * (d->ny - 1) * d->dy,
                   is3 ? d->oz - 0.5 * (d->nz - 1) * d->dz : 0.0};
@@ -181,8 +182,11 @@ ct_status_t ctsf_build_views(const ct_geom_desc_t *d, ct_geom *g)
             o.lane_stride = std::max(stride, 1);
             o.ek = (float)(hk_max * 1.10 + 0.05);
             o.el = (float)(is3 ? hl_max * 1.10 + 0.05 : 0.0);
+            // columns / rows one footprint can span: floor(kc+t3) - floor(kc+t0) + 1 <= 2 ek + 2
+            if (2.0 * o.ek + 2.0 > 6.0 || 2.0 * o.el + 2.0 > 8.0) small_fp = 0;
             g->h_fp[i] = o;
         }
     }
+    g->fp_hoist_ok = (is3 && g->all_untilted && small_fp) ? 1 : 0;
     return CT_OK;
 }

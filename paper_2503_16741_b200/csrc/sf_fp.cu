@@ -69,6 +69,7 @@ constexpr int FPW = 8;            // warps per CTA
 constexpr int FMINB = 3;          // CTAs per SM the register budget is sized for
 constexpr int FTK = 64;           // cells per warp tile
 constexpr int FTL = 32;           // rows per warp tile (3-D)
+constexpr int FKR = 6;            // untilted fast path: F1 weights of up to FKR columns live in registers
 constexpr int FLM = 4;            // pad rows: the first FLM footprint rows are updated unconditionally
 constexpr unsigned FULL = 0xffffffffu;
 
@@ -99,7 +100,7 @@ __device__ __forceinline__ void fp_round_rows(uint32_t ca, float w, const float 
     }
 }
 
-template <int DIM, int ARC, int NB>
+template <int DIM, int ARC, int NB, int UNT>
 __global__ void __launch_bounds__(32 * FPW, FMINB)
 fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ vol,
                const float *__restrict__ volT, float *__restrict__ proj, int view_begin, int view_stride,
@@ -208,6 +209,118 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
         const float q = (float)iq;
         const float aq0 = fmaf(q, v.aq, v.a0), bq0 = fmaf(q, v.bq, v.b0), cq0 = fmaf(q, v.cq, v.c0);
         const float *slab = src + (size_t)iq * np;
+
+        if (UNT) {
+            // ---- untilted frames with small footprints (n.z = u.z = 0; K <= FKR columns, L <= 2 FLM rows) ---
+            // Lanes keep their p while the warp walks the region's rows: the whole transaxial part (trapezoid,
+            // column range, conflict check, the F1 weights themselves) is computed once per (p, q) and held in
+            // registers; a pass is left with the axial rectangle, the amplitude and K rounds of pure updates.
+            for (int col = 0; col < sp; ++col) {
+                const int nprc = (npr - col + sp - 1) / sp;
+                if (nprc <= 0) break;
+                for (int c0 = 0; c0 < nprc; c0 += 32) {
+                    const int pi = c0 + lane;
+                    const bool actp = pi < nprc;
+                    const int ip = actp ? p_lo + col + sp * pi : p_lo;
+                    const int sh = __float2int_rn(sigma * (float)(ip - p_lo));
+                    const float p = (float)ip;
+                    const float a = fmaf(p, v_ap, aq0), b = fmaf(p, v_bp, bq0), cpq = fmaf(p, v_cp, cq0);
+                    const float inv_a = rcp_nr(a);
+                    SfTrans T;
+                    sf_transaxial<ARC>(v, a, b, inv_a, T);
+                    const int k_lo = (int)floorf(T.kc + T.t0);
+                    const int k_hi = (int)floorf(T.kc + T.t3);
+                    const bool livek = actp && k_hi >= k0 && k_lo <= k_top;
+                    const int j_a = livek ? max(0, k0 - k_lo) : 0;
+                    const int j_b = livek ? min(k_hi, k_top) - k_lo : -1;
+                    if (__reduce_max_sync(FULL, j_b + 1) == 0) continue;
+                    const unsigned same = __match_any_sync(FULL, livek ? k_lo : INT_MIN + lane) & ~(1u << lane);
+                    const bool ok = __all_sync(FULL, same == 0u);
+                    float f1[FKR];                       // weight of column k_lo + j
+                    {
+                        float xi = (float)k_lo - T.kc, g0 = sf_G(T, xi);
+#pragma unroll
+                        for (int j = 0; j < FKR; ++j) {
+                            xi += 1.0f;
+                            const float g1 = sf_G(T, xi);
+                            f1[j] = g1 - g0;
+                            g0 = g1;
+                        }
+                    }
+                    // z-independent parts of the axial rectangle and of the amplitude
+                    const float n2ab = fmaf(a, a, b * b);
+                    const float Rg = ARC ? v.Rv * rsqrt_nr(n2ab) : v.Rv * inv_a;
+                    const float half = fabsf(Rg * v.hcz);
+                    const float m = fmaxf(fabsf(p + v.ep0), fabsf(q + v.eq0));
+                    const float m2 = m * m;
+                    int ca_k = (int)smem_addr(tile) + 4 * (livek ? k_lo - k0 : 0);            // row 0, column k_lo
+                    asm volatile("" : "+r"(ca_k));          // keep it in a register: ptxas otherwise rebuilds it per round
+                    const float *xcol = slab + ip;
+                    const int n_serial = ok ? 1 : 32;       // !ok: one lane at a time (never expected)
+                    for (int r = 0; r < nrows; ++r) {
+                        const int izr = zs_lo + r + sh;
+                        const bool act = livek && izr >= 0 && izr < nz;
+                        const int iz = act ? izr : 0;
+                        const float x = __ldg(xcol + (unsigned)(iz * zstride));
+                        const float c = fmaf((float)iz, v_cz, cpq);
+                        SfAxial A;
+                        A.lc = fmaf(Rg, c, v.lv0); A.tlo = -half; A.thi = half;
+                        const int l_lo = max(l0, (int)floorf(A.lc - half));
+                        const int l_hi = min(l_top, (int)floorf(A.lc + half));
+                        const bool live = act && l_lo <= l_hi;
+                        if (!__any_sync(FULL, live)) continue;
+                        const int L = live ? l_hi - l_lo + 1 : 0;
+                        const int Lmax = __reduce_max_sync(FULL, L);
+                        const float n2 = fmaf(c, c, n2ab);
+                        const float ax = x * n2 * rsqrt_approx(n2 * m2);
+                        float f2[2 * FLM];
+                        if (Lmax > FLM) sf_F2_run<2 * FLM>(A, (float)l_lo, f2);
+                        else            sf_F2_run<FLM>(A, (float)l_lo, f2);
+                        const uint32_t ca = (uint32_t)(ca_k + 4 * FTK * (live ? l_lo - l0 : 0));
+                        const int Kall = __reduce_max_sync(FULL, live ? j_b + 1 : 0);
+                        for (int ser = 0; ser < n_serial; ++ser) {
+                            const bool mine = live && (ok || lane == ser);
+                            if (Lmax <= FLM) {
+#pragma unroll
+                                for (int jk = 0; jk < FKR; ++jk) {
+                                    if (jk >= Kall) break;               // warp-uniform
+                                    if (mine && jk >= j_a && jk <= j_b)
+                                        fp_round_rows<true, false>(ca + 4u * jk, f1[jk] * ax, f2, L);
+                                    __syncwarp();
+                                }
+                            } else {
+#pragma unroll
+                                for (int jk = 0; jk < FKR; ++jk) {
+                                    if (jk >= Kall) break;               // warp-uniform
+                                    if (mine && jk >= j_a && jk <= j_b)
+                                        fp_round_rows<true, true>(ca + 4u * jk, f1[jk] * ax, f2, L);
+                                    __syncwarp();
+                                }
+                            }
+                            // footprints beyond the host's bound (never expected): columns >= FKR and rows >= 2 FLM
+                            // with weights evaluated on the fly
+                            if (Kall > FKR || Lmax > 2 * FLM) {
+                                for (int lb = 0; lb < Lmax; lb += 2 * FLM) {
+                                    float g2[2 * FLM];
+                                    sf_F2_run<2 * FLM>(A, (float)(l_lo + lb), g2);
+                                    SfTrans T2;                  // recomputed here so that T need not stay live
+                                    sf_transaxial<ARC>(v, a, b, inv_a, T2);
+                                    for (int jk = (lb == 0 ? FKR : 0); jk < Kall; ++jk) {
+                                        if (mine && jk >= j_a && jk <= j_b) {
+                                            const float xi = (float)(k_lo + jk) - T2.kc;
+                                            const float w = (sf_G(T2, xi + 1.0f) - sf_G(T2, xi)) * ax;
+                                            fp_round_rows<false, true>(ca + 4u * jk + 4u * FTK * lb, w, g2, L - lb);
+                                        }
+                                        __syncwarp();
+                                    }
+                                }
+                            }
+                        }
+                    }
+                }
+            }
+            continue;
+        }
 
         for (int col = 0; col < sp; ++col) {
             const int nprc = (npr - col + sp - 1) / sp;
@@ -347,7 +460,8 @@ void launch_fp(const ct_geom *g, const float *d_vol, const float *d_volT, float 
     const size_t vbs = (size_t)pr.nx * pr.ny * pr.nz, pbs = (size_t)vc * pr.nv * pr.nu;
     constexpr int ROWS = DIM == 3 ? FTL + FLM : NB;
     const size_t smem = (size_t)FPW * ROWS * FTK * sizeof(float);
-    auto kern = fp_band_kernel<DIM, ARC, NB>;
+    auto kern = (DIM == 3 && g->fp_hoist_ok && !getenv("CTSF_FP_NOHOIST")) ? fp_band_kernel<DIM, ARC, NB, DIM == 3 ? 1 : 0>
+                                                                            : fp_band_kernel<DIM, ARC, NB, 0>;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const long n_items = (long)tiles_k * bands_l * ((vc + FPW - 1) / FPW) * FPW;
     // testing aid: CTSF_FP_PAD=<voxels> widens the swept voxel region; the result must not change beyond
