@@ -283,6 +283,103 @@ int sfo_bp(const sfo_geom *g, const double *proj, const int *views, int n_sel, d
     return nthreads;
 }
 
+/* ---- "recon" mode ("depth-dependent weighting specifically for FBP
+ * reconstruction", "discrete ramp filter").  The paper prints neither formula; DESIGN.md
+ * readings R23 (backprojection) and R24 (filter) are followed step by step.  Pins: tests/test_oracle_recon.py
+ * (filtered backprojection of analytic disk / sphere projections returns the attenuation value). ------- */
+
+/* R24: q = du * sum_m p'[m] h[k-m] along every detector row of the selected views.
+ * p' = p * R/sqrt(R^2 + s^2 + t^2) (flat; (s,t) measured from the foot of the source normal) or
+ * p * cos(gamma) * R/sqrt(R^2 + t^2) (arc; gamma = u_k/R).  h[0] = 1/(4 du^2), h[even] = 0,
+ * h[odd n] = -1/(pi n du)^2 (flat), -1/(pi R sin(n du/R))^2 (arc).  proj, out: [n_sel][nv][nu]. */
+int sfo_fbp_filter(const sfo_geom *g, const double *proj, const int *views, int n_sel, double *out)
+{
+    const double PI = 3.14159265358979323846;
+    for (int j = 0; j < n_sel; ++j) {
+        sfo_frame f; make_frame(g, views[j], &f);
+        double *pw = malloc(sizeof(double) * g->nu);
+        for (int l = 0; l < g->nv; ++l) {
+            const double *p = proj + ((size_t)j*g->nv + l)*g->nu;
+            double *q = out + ((size_t)j*g->nv + l)*g->nu;
+            double t = g->dim == 3 ? (l - 0.5*(g->nv - 1))*g->dv + f.Dv : 0.0;
+            for (int k = 0; k < g->nu; ++k) {
+                double uk = (k - 0.5*(g->nu - 1))*g->du;
+                if (g->det_type == 0) { double s = uk + f.Du; pw[k] = p[k] * f.R / sqrt(f.R*f.R + s*s + t*t); }
+                else                  { pw[k] = p[k] * cos(uk / f.R) * f.R / sqrt(f.R*f.R + t*t); }
+            }
+            for (int k = 0; k < g->nu; ++k) {
+                double acc = 0.0;
+                for (int m = 0; m < g->nu; ++m) {
+                    int n = k - m; if (n < 0) n = -n;
+                    double h;
+                    if (n == 0) h = 1.0 / (4.0*g->du*g->du);
+                    else if (n % 2 == 0) h = 0.0;
+                    else if (g->det_type == 0) h = -1.0 / (PI*n*g->du * PI*n*g->du);
+                    else { double sn = PI * f.R * sin(n*g->du / f.R); h = -1.0 / (sn*sn); }
+                    acc += pw[m] * h;
+                }
+                q[k] = g->du * acc;
+            }
+        }
+        free(pw);
+    }
+    return 0;
+}
+
+/* R23, one voxel: sum over views of W * sum_kl (F1/sumF1)(F2/sumF2) q, W = d R / a^2 (flat),
+ * d R / (a^2 + b^2) (arc); d = in-plane distance of the rotation centre (world origin) from the
+ * source: -S.n (flat), sqrt((S.n)^2 + (S.u)^2) (arc).  sumF1, sumF2: unclipped footprint sums. */
+static double bp_voxel_recon(const sfo_geom *g, const sfo_frame *frames, const double *q, int n_sel,
+                             int ix, int iy, int iz, double *F1, double *F2)
+{
+    const size_t ncell = (size_t)g->nu * g->nv;
+    double Pc[3] = { g->ox + (ix - 0.5*(g->nx - 1))*g->dx, g->oy + (iy - 0.5*(g->ny - 1))*g->dy,
+                     g->dim == 3 ? g->oz + (iz - 0.5*(g->nz - 1))*g->dz : 0.0 };
+    double acc = 0.0;
+    for (int j = 0; j < n_sel; ++j) {
+        const sfo_frame *f = &frames[j];
+        int klo, khi, llo, lhi; double amp, tau[4];
+        if (!footprint(g, f, ix, iy, iz, &klo, &khi, F1, &llo, &lhi, F2, &amp, tau)) continue;
+        double sumF1 = 0.5*(tau[3] + tau[2] - tau[1] - tau[0]) / g->du, sumF2 = 1.0;
+        if (g->dim == 3) {
+            double Pm[3] = { Pc[0], Pc[1], Pc[2] - 0.5*g->dz }, Pp[3] = { Pc[0], Pc[1], Pc[2] + 0.5*g->dz };
+            double s_unused, ta, tb;
+            det_coords(g, f, Pm, &s_unused, &ta); det_coords(g, f, Pp, &s_unused, &tb);
+            sumF2 = fabs(tb - ta) / g->dv;
+        }
+        double w[3] = { Pc[0]-f->S[0], Pc[1]-f->S[1], Pc[2]-f->S[2] };
+        double a = dot3(w, f->n), b = dot3(w, f->u);
+        double Sn = dot3(f->S, f->n), Su = dot3(f->S, f->u);
+        double W = g->det_type == 0 ? (-Sn) * f->R / (a*a) : sqrt(Sn*Sn + Su*Su) * f->R / (a*a + b*b);
+        double sum = 0.0;
+        const double *y = q + ncell*j;
+        for (int l = llo; l <= lhi; ++l)
+            for (int k = klo; k <= khi; ++k)
+                sum += F1[k - klo] * F2[l - llo] * y[(size_t)l*g->nu + k];
+        acc += W * sum / (sumF1 * sumF2);
+    }
+    return acc;
+}
+
+/* vol = B q over the selected views (recon-mode backprojection).  q [n_sel][nv][nu]; vol overwritten. */
+int sfo_bp_recon(const sfo_geom *g, const double *q, const int *views, int n_sel, double *vol)
+{
+    sfo_frame *frames = malloc(sizeof(sfo_frame) * (n_sel > 0 ? n_sel : 1));
+    for (int j = 0; j < n_sel; ++j) make_frame(g, views[j], &frames[j]);
+    #pragma omp parallel
+    {
+        double *F1 = malloc(sizeof(double)*g->nu), *F2 = malloc(sizeof(double)*g->nv);
+        #pragma omp for schedule(dynamic, 4) collapse(2)
+        for (int iz = 0; iz < g->nz; ++iz)
+            for (int iy = 0; iy < g->ny; ++iy)
+                for (int ix = 0; ix < g->nx; ++ix)
+                    vol[((size_t)iz*g->ny + iy)*g->nx + ix] = bp_voxel_recon(g, frames, q, n_sel, ix, iy, iz, F1, F2);
+        free(F1); free(F2);
+    }
+    free(frames);
+    return 0;
+}
+
 /* (A^T y) at n listed voxels (ijk[3*i..] = ix, iy, iz), all views; y is the FULL [n_views][nv][nu]. */
 int sfo_bp_voxels(const sfo_geom *g, const double *proj, const int *ijk, int n, double *out)
 {

@@ -52,6 +52,8 @@ def _load():
         lib.sfo_det_coords.argtypes = [P, I, P, P]
         lib.sfo_fp.argtypes = [P, P, P, I, P]
         lib.sfo_bp.argtypes = [P, P, P, I, P]
+        lib.sfo_fbp_filter.argtypes = [P, P, P, I, P]
+        lib.sfo_bp_recon.argtypes = [P, P, P, I, P]
         lib.sfo_bp_voxels.argtypes = [P, P, P, I, P]
         lib.sfo_bp_voxels_f32.argtypes = [P, P, P, I, P]
         _lib = lib
@@ -149,6 +151,31 @@ class Oracle:
         for b in range(p.shape[0]):
             self.threads = self.lib.sfo_bp(ctypes.byref(self.g), p[b].ctypes.data, views.ctypes.data,
                                            len(views), out[b].ctypes.data)
+        return out.reshape(lead + (self.nz, self.ny, self.nx))
+
+    def fbp_filter(self, proj, views=None):
+        """Recon mode, reading R24: cosine pre-weight + discrete ramp filter along u.
+        proj [..., n_sel, nv, nu] -> same shape, float64."""
+        views = self._views(views)
+        proj = _f64(proj)
+        p = proj.reshape((-1, len(views), self.nv, self.nu))
+        out = np.empty_like(p)
+        for b in range(p.shape[0]):
+            self.lib.sfo_fbp_filter(ctypes.byref(self.g), p[b].ctypes.data, views.ctypes.data, len(views),
+                                    out[b].ctypes.data)
+        return out.reshape(proj.shape)
+
+    def bp_recon(self, q, views=None):
+        """Recon mode, reading R23: x = B q (normalised footprints x depth weight d R / a^2).
+        q [..., n_sel, nv, nu]; returns [..., nz, ny, nx] float64."""
+        views = self._views(views)
+        q = _f64(q)
+        lead = q.shape[:-3] if q.ndim > 3 else ()
+        p = q.reshape((-1, len(views), self.nv, self.nu))
+        out = np.empty((p.shape[0], self.nz, self.ny, self.nx))
+        for b in range(p.shape[0]):
+            self.lib.sfo_bp_recon(ctypes.byref(self.g), p[b].ctypes.data, views.ctypes.data, len(views),
+                                  out[b].ctypes.data)
         return out.reshape(lead + (self.nz, self.ny, self.nx))
 
     def bp_voxels(self, proj, ijk):

@@ -1,0 +1,109 @@
+"""Pins for the oracle's "recon" mode (readings R23, R24): filtered
+backprojection x = (pi/N) B(filter(p)) of ANALYTIC projections (closed-form chord lengths, cell-centre rays --
+nothing computed by a projector) must return the attenuation value inside a uniform object.  Fan-beam FBP and
+the mid-plane of circular cone-beam FDK are exact inversions, so the only error is discretisation; a dropped
+cosine weight, a wrong filter scale, a missing (pi/N) or a wrong depth weight each shift the plateau by >= 3 %.
+CPU only (-m "not gpu")."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle.sf_oracle import Oracle
+from paper_2503_16741_b200 import workloads as W
+
+MU = 0.02
+
+
+def _rays(c):
+    """Unit ray directions through every cell centre: [n_views, nv, nu, 3] and the sources [n_views, 3]."""
+    nu, nv, du, dv = c["nu"], c["nv"], c["du"], c["dv"]
+    u = (np.arange(nu) - 0.5 * (nu - 1)) * du
+    v = (np.arange(nv) - 0.5 * (nv - 1)) * dv
+    S, D, eu, ev = c["src"], c["det_center"], c["det_u"], c["det_v"]
+    out = np.empty((len(S), nv, nu, 3))
+    for i in range(len(S)):
+        n = np.cross(eu[i], ev[i])
+        if np.dot(D[i] - S[i], n) < 0:
+            n = -n
+        R = np.dot(D[i] - S[i], n)
+        if c["det_type"] == "flat":
+            P = D[i][None, None, :] + u[None, :, None] * eu[i] + v[:, None, None] * ev[i]
+        else:
+            g = u / R
+            P = (S[i][None, None, :] + R * (np.sin(g)[None, :, None] * eu[i] + np.cos(g)[None, :, None] * n)
+                 + (v[:, None, None] + np.dot(D[i] - S[i], ev[i])) * ev[i])
+        d = P - S[i]
+        out[i] = d / np.linalg.norm(d, axis=-1, keepdims=True)
+    return out, S
+
+
+def _ball_projections(c, radius, centre):
+    """mu * chord length of the rays through a uniform ball (3-D) / disk (2-D, z ignored)."""
+    dirs, S = _rays(c)
+    oc = S[:, None, None, :] - np.asarray(centre)[None, None, None, :]
+    if c["dim"] == 2:
+        dirs = dirs.copy(); dirs[..., 2] = 0.0
+        dirs /= np.linalg.norm(dirs, axis=-1, keepdims=True)
+        oc = oc.copy(); oc[..., 2] = 0.0
+    b = np.sum(oc * dirs, axis=-1)
+    disc = b * b - (np.sum(oc * oc, axis=-1) - radius ** 2)
+    return MU * 2.0 * np.sqrt(np.maximum(disc, 0.0))
+
+
+def _fbp(c, p):
+    o = Oracle(W.geom_keys(c))
+    q = o.fbp_filter(p)
+    return (math.pi / c["n_views"]) * o.bp_recon(q)
+
+
+@pytest.mark.parametrize("index,shrink", [(1, dict(nx=64, ny=64, nu=160, n_views=180)),
+                                          (5, dict(nx=96, ny=96, nu=220, n_views=240, batch=1))])
+def test_fan_beam_fbp_of_a_disk(index, shrink):
+    c = W.make_config(index, **shrink)
+    L = c["nx"] * c["dx"]
+    centre, radius = (0.11 * L, -0.07 * L, 0.0), 0.22 * L
+    x = _fbp(c, _ball_projections(c, radius, centre))[0]
+    xs = (np.arange(c["nx"]) - 0.5 * (c["nx"] - 1)) * c["dx"]
+    X, Y = np.meshgrid(xs, xs)
+    r = np.hypot(X - centre[0], Y - centre[1])
+    inside, outside = r < 0.8 * radius, (r > 1.25 * radius) & (np.hypot(X, Y) < 0.45 * L)
+    assert abs(x[inside].mean() / MU - 1.0) < 5e-3, x[inside].mean() / MU
+    assert np.abs(x[inside] / MU - 1.0).max() < 3e-2
+    assert abs(x[outside].mean()) < 1e-2 * MU
+
+
+@pytest.mark.parametrize("index,shrink", [(2, dict(nx=40, ny=40, nz=24, nu=96, nv=64, n_views=120)),
+                                          (3, dict(nx=48, ny=48, nz=12, nu=120, nv=24, n_views=144))])
+def test_cone_beam_fdk_of_a_ball_mid_plane(index, shrink):
+    c = W.make_config(index, **shrink)
+    Lx, Lz = c["nx"] * c["dx"], c["nz"] * c["dz"]
+    radius = min(0.25 * Lx, 0.35 * Lz)
+    centre = (0.08 * Lx, -0.05 * Lx, 0.0)
+    x = _fbp(c, _ball_projections(c, radius, centre))
+    xs = (np.arange(c["nx"]) - 0.5 * (c["nx"] - 1)) * c["dx"]
+    X, Y = np.meshgrid(xs, xs)
+    r = np.hypot(X - centre[0], Y - centre[1])
+    inside = r < 0.75 * radius
+    mid = 0.5 * (x[c["nz"] // 2 - 1] + x[c["nz"] // 2])           # the two slices next to z = 0
+    assert abs(mid[inside].mean() / MU - 1.0) < 1e-2, mid[inside].mean() / MU
+    assert np.abs(mid[inside] / MU - 1.0).max() < 4e-2
+
+
+def test_recon_backprojection_weights_are_normalised():
+    """R23: with q == 1 and the footprint fully on the detector, B q at a voxel is sum_views d R / a^2
+    exactly (the footprint is a normalised interpolation kernel)."""
+    c = W.make_config(2, nx=9, ny=9, nz=7, nu=64, nv=64, n_views=5)
+    o = Oracle(W.geom_keys(c))
+    x = o.bp_recon(np.ones((5, 64, 64)))
+    ix, iy, iz = 6, 3, 4
+    P = np.array([(ix - 4) * c["dx"], (iy - 4) * c["dy"], (iz - 3) * c["dz"]])
+    want = 0.0
+    for i in range(5):
+        n = np.cross(c["det_u"][i], c["det_v"][i])
+        if np.dot(c["det_center"][i] - c["src"][i], n) < 0:
+            n = -n
+        R = np.dot(c["det_center"][i] - c["src"][i], n)
+        a = np.dot(P - c["src"][i], n)
+        want += np.dot(-c["src"][i], n) * R / a ** 2
+    assert abs(x[iz, iy, ix] / want - 1.0) < 1e-12
