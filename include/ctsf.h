@@ -96,6 +96,26 @@ CTSF_API ct_status_t ct_fp_sf_views(const ct_geom_t *geom, const float *d_vol, f
 CTSF_API ct_status_t ct_bp_sf_views(const ct_geom_t *geom, const float *d_proj, float *d_vol, int32_t batch,
                            int32_t view_begin, int32_t view_stride, int32_t view_count, ct_stream_t stream);
 
+/* "recon" mode ("the backprojection used in FBP reconstruction differs slightly from the general
+ * backprojection by incorporating a depth-dependent weighting ... 'recon' mode"; "discrete ramp
+ * filter").  The paper prints neither formula; readings R23, R24 define them:
+ *   ct_fbp_filter : q = du * (p' * h) along the channels of every row, p' the cosine-weighted projection,
+ *                   h the band-limited ramp at the channel pitch (flat) / its equi-angular form (arc).
+ *                   d_proj read, d_out written, both DEVICE [batch][views][nv][nu]; NOT in place.
+ *   ct_bp_sf_recon: x[n] = sum_i (d_i R_i / a^2) sum_kl F1(k) F2(l) q[i,l,k] / (sum F1 sum F2): the SF footprint as
+ *                   a normalised interpolation kernel times the depth weight (arc: a^2 -> a^2 + b^2);
+ *                   d_i = distance from the source to the rotation centre (the world origin).
+ * Filtered backprojection of N equi-angular views over 360 degrees: x = (pi / N) * ct_bp_sf_recon(ct_fbp_filter(p)).
+ * Same layouts, overwrite semantics, stream behaviour and errors as ct_bp_sf; *_views take ordered subsets. */
+CTSF_API ct_status_t ct_fbp_filter(const ct_geom_t *geom, const float *d_proj, float *d_out,
+                          int32_t batch, ct_stream_t stream);
+CTSF_API ct_status_t ct_fbp_filter_views(const ct_geom_t *geom, const float *d_proj, float *d_out, int32_t batch,
+                                int32_t view_begin, int32_t view_stride, int32_t view_count, ct_stream_t stream);
+CTSF_API ct_status_t ct_bp_sf_recon(const ct_geom_t *geom, const float *d_proj, float *d_vol,
+                           int32_t batch, ct_stream_t stream);
+CTSF_API ct_status_t ct_bp_sf_recon_views(const ct_geom_t *geom, const float *d_proj, float *d_vol, int32_t batch,
+                                 int32_t view_begin, int32_t view_stride, int32_t view_count, ct_stream_t stream);
+
 /* End-to-end convenience with HOST buffers (pageable or pinned): allocates device buffers from the
  * stream-ordered pool, copies the input host->device, runs the operator, copies the result
  * device->host and synchronises `stream` before returning.  Same layouts as above. */

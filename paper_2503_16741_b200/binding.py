@@ -16,7 +16,8 @@ CT_OK = 0
 STATUS_NAMES = {0: "CT_OK", 1: "CT_ERR_INVALID_ARG", 2: "CT_ERR_GEOMETRY", 3: "CT_ERR_UNSUPPORTED",
                 4: "CT_ERR_ALLOC", 5: "CT_ERR_CUDA"}
 EXPORTS = ("ct_geom_create", "ct_geom_destroy", "ct_fp_sf", "ct_bp_sf", "ct_fp_sf_views", "ct_bp_sf_views",
-           "ct_fp_sf_host", "ct_bp_sf_host", "ct_last_launch_count", "ct_status_string")
+           "ct_fp_sf_host", "ct_bp_sf_host", "ct_fbp_filter", "ct_fbp_filter_views", "ct_bp_sf_recon",
+           "ct_bp_sf_recon_views", "ct_last_launch_count", "ct_status_string")
 
 
 class CtError(RuntimeError):
@@ -56,11 +57,15 @@ def lib():
         L.ct_bp_sf_views.argtypes = [P, P, P, I, I, I, I, P]
         L.ct_fp_sf_host.argtypes = [P, P, P, I, P]
         L.ct_bp_sf_host.argtypes = [P, P, P, I, P]
+        L.ct_fbp_filter.argtypes = [P, P, P, I, P]
+        L.ct_bp_sf_recon.argtypes = [P, P, P, I, P]
+        L.ct_fbp_filter_views.argtypes = [P, P, P, I, I, I, I, P]
+        L.ct_bp_sf_recon_views.argtypes = [P, P, P, I, I, I, I, P]
         L.ct_last_launch_count.argtypes = [P]
         L.ct_last_launch_count.restype = I
         L.ct_status_string.argtypes = [ctypes.c_int]
         L.ct_status_string.restype = ctypes.c_char_p
-        for name in EXPORTS[:8]:
+        for name in EXPORTS[:12]:
             getattr(L, name).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -128,6 +133,24 @@ def ct_fp_sf_host(handle, h_vol, h_proj, batch, stream=0):
 
 def ct_bp_sf_host(handle, h_proj, h_vol, batch, stream=0):
     _check(lib().ct_bp_sf_host(handle, h_proj, h_vol, int(batch), stream), "ct_bp_sf_host")
+
+
+def ct_fbp_filter_views(handle, d_proj, d_out, batch, view_begin, view_stride, view_count, stream=0):
+    _check(lib().ct_fbp_filter_views(handle, d_proj, d_out, batch, view_begin, view_stride, view_count, stream),
+           "ct_fbp_filter_views")
+
+
+def ct_bp_sf_recon_views(handle, d_proj, d_vol, batch, view_begin, view_stride, view_count, stream=0):
+    _check(lib().ct_bp_sf_recon_views(handle, d_proj, d_vol, batch, view_begin, view_stride, view_count, stream),
+           "ct_bp_sf_recon_views")
+
+
+def ct_fbp_filter(handle, d_proj, d_out, batch, stream=0):
+    _check(lib().ct_fbp_filter(handle, d_proj, d_out, batch, stream), "ct_fbp_filter")
+
+
+def ct_bp_sf_recon(handle, d_proj, d_vol, batch, stream=0):
+    _check(lib().ct_bp_sf_recon(handle, d_proj, d_vol, batch, stream), "ct_bp_sf_recon")
 
 
 def ct_last_launch_count(handle):

@@ -86,6 +86,8 @@ ct_status_t ct_geom_create(const ct_geom_desc_t *d, ct_geom_t **out)
     ct_geom *g = new (std::nothrow) ct_geom;
     if (!g) return CT_ERR_ALLOC;
     g->prob = SfProblem{d->dim, d->det_type, d->nx, d->ny, d->nz, d->nu, d->nv, d->n_views};
+    g->du = d->du;
+    g->dv = d->dim == 3 ? d->dv : 1.0;
     ct_status_t st;
     try {
         st = ctsf_build_views(d, g);
@@ -149,6 +151,41 @@ ct_status_t ct_bp_sf_views(const ct_geom_t *g, const float *d_proj, float *d_vol
     if (n < 0) return CT_ERR_CUDA;
     const_cast<ct_geom *>(g)->last_launches.store(n);
     return CT_OK;
+}
+
+ct_status_t ct_bp_sf_recon_views(const ct_geom_t *g, const float *d_proj, float *d_vol, int32_t batch,
+                                 int32_t vb, int32_t vs, int32_t vc, ct_stream_t stream)
+{
+    ct_status_t st = check_call(g, d_proj, d_vol, batch, vb, vs, vc);
+    if (st != CT_OK) return st;
+    int n = ctsf_launch_bp(g, d_proj, d_vol, batch, vb, vs, vc, stream, 0, 1);
+    if (n < 0) return CT_ERR_CUDA;
+    const_cast<ct_geom *>(g)->last_launches.store(n);
+    return CT_OK;
+}
+
+ct_status_t ct_bp_sf_recon(const ct_geom_t *g, const float *d_proj, float *d_vol, int32_t batch, ct_stream_t stream)
+{
+    if (!g) return CT_ERR_INVALID_ARG;
+    return ct_bp_sf_recon_views(g, d_proj, d_vol, batch, 0, 1, g->prob.n_views, stream);
+}
+
+ct_status_t ct_fbp_filter_views(const ct_geom_t *g, const float *d_proj, float *d_out, int32_t batch,
+                                int32_t vb, int32_t vs, int32_t vc, ct_stream_t stream)
+{
+    ct_status_t st = check_call(g, d_proj, d_out, batch, vb, vs, vc);
+    if (st != CT_OK) return st;
+    if (d_proj == d_out) return CT_ERR_INVALID_ARG;           // not in place: every output reads the whole row
+    int n = ctsf_launch_filter(g, d_proj, d_out, batch, vb, vs, vc, stream);
+    if (n < 0) return CT_ERR_CUDA;
+    const_cast<ct_geom *>(g)->last_launches.store(n);
+    return CT_OK;
+}
+
+ct_status_t ct_fbp_filter(const ct_geom_t *g, const float *d_proj, float *d_out, int32_t batch, ct_stream_t stream)
+{
+    if (!g) return CT_ERR_INVALID_ARG;
+    return ct_fbp_filter_views(g, d_proj, d_out, batch, 0, 1, g->prob.n_views, stream);
 }
 
 ct_status_t ct_fp_sf(const ct_geom_t *g, const float *d_vol, float *d_proj, int32_t batch, ct_stream_t stream)

@@ -8,6 +8,7 @@
 
 struct ct_geom {
     SfProblem prob;
+    double du = 1.0, dv = 1.0;        // detector pitches, mm (ramp filter)
     std::vector<SfView> h_bp, h_fp;   // host copies (natural order / forward order with xy swaps)
     SfView *d_bp = nullptr, *d_fp = nullptr;
     int any_swap = 0;                 // some forward view reads the volume through its transpose
@@ -29,8 +30,12 @@ ct_status_t ctsf_build_views(const ct_geom_desc_t *desc, ct_geom *g);
 
 // sf_bp.cu / sf_fp.cu: launchers.  Projection buffers hold `view_count` views; view j of the buffer
 // is geometry view view_begin + j*view_stride.  Return the number of kernels launched, or -1.
-// accumulate != 0 (3-D only): add to d_vol instead of overwriting it.
+// accumulate != 0 (3-D only): add to d_vol instead of overwriting it.  recon != 0: recon-mode weights (R23).
 int ctsf_launch_bp(const ct_geom *g, const float *d_proj, float *d_vol, int batch,
-                   int view_begin, int view_stride, int view_count, void *stream, int accumulate = 0);
+                   int view_begin, int view_stride, int view_count, void *stream, int accumulate = 0,
+                   int recon = 0);
+// sf_filter.cu: cosine pre-weight + discrete ramp filter of the selected views (reading R24).
+int ctsf_launch_filter(const ct_geom *g, const float *d_proj, float *d_out, int batch,
+                       int view_begin, int view_stride, int view_count, void *stream);
 int ctsf_launch_fp(const ct_geom *g, const float *d_vol, float *d_proj, int batch,
                    int view_begin, int view_stride, int view_count, void *stream);

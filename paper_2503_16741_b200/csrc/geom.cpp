@@ -110,6 +110,11 @@ ct_status_t ctsf_build_views(const ct_geom_desc_t *d, ct_geom *g)
             o.qa = (float)(0.5 * (m.ap - m.aq)); o.qb = (float)(0.5 * (m.bp - m.bq));
             o.haz = (float)(0.5 * m.az); o.hbz = (float)(0.5 * m.bz); o.hcz = (float)(0.5 * m.cz);
             o.untilted = untilted ? 1 : 0;
+            {   // recon mode: depth weight numerator d * R (flat: d = -S.n; arc: in-plane distance of the origin)
+                const V3 Sv = S;
+                const double Sn = dot(Sv, n), Su = dot(Sv, u);
+                o.recon_dR = (float)((d->det_type == 0 ? -Sn : std::sqrt(Sn * Sn + Su * Su)) * R);
+            }
             o.swap_xy = sw ? 1 : 0;
             if (pass == 0) g->h_bp[i] = o;
 

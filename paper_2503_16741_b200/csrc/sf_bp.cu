@@ -29,7 +29,7 @@ namespace {
 // ---------------------------------------------------------------------------------------------------
 constexpr int BP_VC = 16;     // views staged per chunk
 
-template <int ARC, int NB>
+template <int ARC, int NB, int RECON>
 __global__ void __launch_bounds__(128)
 bp_pixel_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ proj,
                 float *__restrict__ vol, int view_begin, int view_stride, int view_count,
@@ -72,7 +72,7 @@ bp_pixel_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
             const int k_lo = max(0, (int)floorf(T.kc + T.t0));
             const int k_hi = min(pr.nu - 1, (int)floorf(T.kc + T.t3));
             if (k_lo > k_hi) continue;
-            const float amp = sf_amplitude(v, a, b, 0.0f, p, q);
+            const float amp = RECON ? sf_recon_weight<ARC>(v, T, 1.0f, a, b) : sf_amplitude(v, a, b, 0.0f, p, q);
             const float *y = proj + (size_t)(v0 + j) * pr.nu;
             float sum[NB];
 #pragma unroll
@@ -206,7 +206,7 @@ __device__ __forceinline__ float gather_tile(const float *__restrict__ tile, con
     return sum;
 }
 
-template <int ARC>
+template <int ARC, int RECON>
 __global__ void __launch_bounds__(BRICK_THREADS, 3)
 bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ proj,
                 const __grid_constant__ CUtensorMap tmap, int use_tma, float *__restrict__ vol,
@@ -323,7 +323,8 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
                             const int l_lo = max(max(0, tl0), (int)floorf(A.lc + A.tlo));
                             const int l_hi = min(min(pr.nv - 1, tl0 + TH - 1), (int)floorf(A.lc + A.thi));
                             if (l_lo > l_hi) continue;
-                            const float amp = sf_amplitude(v, a, b, c, p, q);
+                            const float amp = RECON ? sf_recon_weight<ARC>(v, T, A.thi - A.tlo, a, b)
+                                                    : sf_amplitude(v, a, b, c, p, q);
                             const float sum = gather_tile(tile, T, A, k_lo, k_hi, l_lo, l_hi, tk0, tl0);
                             float *ap = accs + zi * BRICK_THREADS + tid;
                             *ap = fmaf(amp, sum, *ap);
@@ -366,7 +367,7 @@ EncodeTiledFn get_encode()
 
 template <int ARC>
 int launch_brick(const ct_geom *g, const float *d_proj, float *d_vol, int batch, int vb, int vs, int vc, cudaStream_t st,
-                 int accumulate)
+                 int accumulate, int recon)
 {
     const SfProblem &pr = g->prob;
     CUtensorMap tmap;
@@ -384,7 +385,7 @@ int launch_brick(const ct_geom *g, const float *d_proj, float *d_vol, int batch,
             use_tma = (dbg && dbg[0] >= '1' && dbg[0] <= '3') ? dbg[0] - '0' : 3;
     }
     const size_t smem = (size_t)(2 * TILE_FLOATS + BZ * BRICK_THREADS) * sizeof(float);
-    auto kern = bp_brick_kernel<ARC>;
+    auto kern = recon ? bp_brick_kernel<ARC, 1> : bp_brick_kernel<ARC, 0>;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const int nbz = (pr.nz + BZ - 1) / BZ;
     int launches = 0;
@@ -416,19 +417,20 @@ int launch_brick(const ct_geom *g, const float *d_proj, float *d_vol, int batch,
 
 template <int ARC, int NB>
 void launch_pixel(const ct_geom *g, const float *d_proj, float *d_vol, int b0, int groups, int vb, int vs, int vc,
-                  cudaStream_t st)
+                  cudaStream_t st, int recon)
 {
     const SfProblem &pr = g->prob;
     const size_t pbs = (size_t)vc * pr.nu, vbs = (size_t)pr.nx * pr.ny;
     dim3 block(16, 8, 1);
     dim3 grid((pr.nx + block.x - 1) / block.x, (pr.ny + block.y - 1) / block.y, groups);
-    bp_pixel_kernel<ARC, NB><<<grid, block, 0, st>>>(pr, g->d_bp, d_proj + (size_t)b0 * pbs, d_vol + (size_t)b0 * vbs,
-                                                     vb, vs, vc, (unsigned)pbs, (unsigned)vbs);
+    auto kern = recon ? bp_pixel_kernel<ARC, NB, 1> : bp_pixel_kernel<ARC, NB, 0>;
+    kern<<<grid, block, 0, st>>>(pr, g->d_bp, d_proj + (size_t)b0 * pbs, d_vol + (size_t)b0 * vbs,
+                                 vb, vs, vc, (unsigned)pbs, (unsigned)vbs);
 }
 
 template <int ARC>
 int launch_pixel_batches(const ct_geom *g, const float *d_proj, float *d_vol, int batch, int vb, int vs, int vc,
-                         cudaStream_t st)
+                         cudaStream_t st, int recon)
 {
     // batch images share the weights (S6): groups of 16, 8, 4, 2, 1 images per thread
     int launches = 0, b0 = 0;
@@ -439,11 +441,11 @@ int launch_pixel_batches(const ct_geom *g, const float *d_proj, float *d_vol, in
         while (groups > 0) {
             const int gnow = groups > 65535 ? 65535 : groups;
             switch (nb) {
-                case 16: launch_pixel<ARC, 16>(g, d_proj, d_vol, b0, gnow, vb, vs, vc, st); break;
-                case 8: launch_pixel<ARC, 8>(g, d_proj, d_vol, b0, gnow, vb, vs, vc, st); break;
-                case 4: launch_pixel<ARC, 4>(g, d_proj, d_vol, b0, gnow, vb, vs, vc, st); break;
-                case 2: launch_pixel<ARC, 2>(g, d_proj, d_vol, b0, gnow, vb, vs, vc, st); break;
-                default: launch_pixel<ARC, 1>(g, d_proj, d_vol, b0, gnow, vb, vs, vc, st); break;
+                case 16: launch_pixel<ARC, 16>(g, d_proj, d_vol, b0, gnow, vb, vs, vc, st, recon); break;
+                case 8: launch_pixel<ARC, 8>(g, d_proj, d_vol, b0, gnow, vb, vs, vc, st, recon); break;
+                case 4: launch_pixel<ARC, 4>(g, d_proj, d_vol, b0, gnow, vb, vs, vc, st, recon); break;
+                case 2: launch_pixel<ARC, 2>(g, d_proj, d_vol, b0, gnow, vb, vs, vc, st, recon); break;
+                default: launch_pixel<ARC, 1>(g, d_proj, d_vol, b0, gnow, vb, vs, vc, st, recon); break;
             }
             ++launches;
             b0 += gnow * nb;
@@ -456,15 +458,15 @@ int launch_pixel_batches(const ct_geom *g, const float *d_proj, float *d_vol, in
 }  // namespace
 
 int ctsf_launch_bp(const ct_geom *g, const float *d_proj, float *d_vol, int batch,
-                   int view_begin, int view_stride, int view_count, void *stream, int accumulate)
+                   int view_begin, int view_stride, int view_count, void *stream, int accumulate, int recon)
 {
     cudaStream_t st = (cudaStream_t)stream;
     const int arc = g->prob.det_type, dim = g->prob.dim;
     if (accumulate && dim != 3) return -1;       // only the 3-D brick kernel can add to its output
     int n;
-    if (dim == 2) n = arc ? launch_pixel_batches<1>(g, d_proj, d_vol, batch, view_begin, view_stride, view_count, st)
-                          : launch_pixel_batches<0>(g, d_proj, d_vol, batch, view_begin, view_stride, view_count, st);
-    else          n = arc ? launch_brick<1>(g, d_proj, d_vol, batch, view_begin, view_stride, view_count, st, accumulate)
-                          : launch_brick<0>(g, d_proj, d_vol, batch, view_begin, view_stride, view_count, st, accumulate);
+    if (dim == 2) n = arc ? launch_pixel_batches<1>(g, d_proj, d_vol, batch, view_begin, view_stride, view_count, st, recon)
+                          : launch_pixel_batches<0>(g, d_proj, d_vol, batch, view_begin, view_stride, view_count, st, recon);
+    else          n = arc ? launch_brick<1>(g, d_proj, d_vol, batch, view_begin, view_stride, view_count, st, accumulate, recon)
+                          : launch_brick<0>(g, d_proj, d_vol, batch, view_begin, view_stride, view_count, st, accumulate, recon);
     return cudaGetLastError() == cudaSuccess ? n : -1;
 }

@@ -36,7 +36,8 @@ struct SfView {
     float ku0c, lv0c;          // detector coordinates (cells) of the point the Dm ray hits
     float ek, el;              // tile expansion (cells / rows): max |footprint half extent| + margin
     int32_t lane_stride;       // voxels p, p + lane_stride project >= 1 cell apart (conflict-free rounds)
-    int32_t pad0, pad1, pad2;
+    float recon_dR;            // recon mode (reading R23): d * R, d = distance source -> rotation centre (world origin)
+    int32_t pad1, pad2;
 };
 
 struct SfProblem {

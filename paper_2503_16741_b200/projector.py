@@ -61,6 +61,32 @@ class Geometry:
                          torch.cuda.current_stream(proj.device).cuda_stream)
         return out.view(lead + self.vol_shape)
 
+    # ---- recon mode (readings R23, R24) --------------------------------
+    def fbp_filter(self, proj, views=None, out=None):
+        """Cosine pre-weight + discrete ramp filter along the channels; proj [..., n_sel, nv, nu] -> same shape."""
+        vb, vs, vc = self._views(views)
+        lead, batch, proj = _prep(proj, (vc,) + self.det_shape)
+        if out is None:
+            out = torch.empty_like(proj)
+        B.ct_fbp_filter_views(self.handle, proj.data_ptr(), out.data_ptr(), batch, vb, vs, vc,
+                              torch.cuda.current_stream(proj.device).cuda_stream)
+        return out.view(lead + (vc,) + self.det_shape)
+
+    def bp_recon(self, proj, views=None, out=None):
+        """Recon-mode backprojection (normalised footprints x depth weight); proj [..., n_sel, nv, nu] -> volume."""
+        vb, vs, vc = self._views(views)
+        lead, batch, proj = _prep(proj, (vc,) + self.det_shape)
+        if out is None:
+            out = torch.empty((batch,) + self.vol_shape, device=proj.device, dtype=torch.float32)
+        B.ct_bp_sf_recon_views(self.handle, proj.data_ptr(), out.data_ptr(), batch, vb, vs, vc,
+                               torch.cuda.current_stream(proj.device).cuda_stream)
+        return out.view(lead + self.vol_shape)
+
+    def fbp(self, proj):
+        """Filtered backprojection of N equi-angular views over 360 degrees: (pi / N) B(filter(p))."""
+        import math
+        return self.bp_recon(self.fbp_filter(proj)).mul_(math.pi / self.n_views)
+
     def last_launch_count(self):
         return B.ct_last_launch_count(self.handle)
 
@@ -109,17 +135,23 @@ class BP(torch.autograd.Function):
 
 class Projector(torch.nn.Module):
     """`A = Projector(geom, 'proj', 'SF', 'forward'); sino = A(img)` (PAPER.md:118-122).
-    Only mode 'proj' and algorithm 'SF' exist here; direction is 'forward' or 'backward'.
+    Algorithm 'SF' only; mode 'proj' (matched pair, differentiable) or 'recon' (FBP backprojection of
+    PAPER.md:103, direction 'backward' only); direction is 'forward' or 'backward'.
     `subset=(view_begin, view_stride, view_count)` restricts to an ordered subset."""
 
     def __init__(self, geom, mode="proj", algo="SF", direction="forward"):
         super().__init__()
-        if mode != "proj" or algo != "SF":
-            raise NotImplementedError("only mode='proj', algo='SF' are built (see DESIGN.md, out of scope)")
+        if mode not in ("proj", "recon") or algo != "SF":
+            raise NotImplementedError("only algo='SF' with mode 'proj' or 'recon' is built (see DESIGN.md)")
         if direction not in ("forward", "backward"):
             raise ValueError(direction)
+        if mode == "recon" and direction != "backward":
+            raise NotImplementedError("'recon' mode is the FBP backprojection: direction must be 'backward'")
+        self.mode = mode
         self.geom = geom if isinstance(geom, Geometry) else Geometry(geom)
         self.direction = direction
 
     def forward(self, x, subset=None):
+        if self.mode == "recon":            # not differentiable: FBP is used for reconstruction only
+            return self.geom.bp_recon(x, subset)
         return (FP if self.direction == "forward" else BP).apply(x, self.geom, subset)
