@@ -146,6 +146,8 @@ def main():
     ap.add_argument("--impl", default="ctsf")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--fbp", action="store_true",
+                    help="also time recon mode (row f2): ct_fbp_filter + ct_bp_sf_recon on the step's projections")
     ap.add_argument("--view-stride", type=int, default=1,
                     help="profiling aid: use every S-th view only (ordered subset); not a bench value")
     args = ap.parse_args()
@@ -221,6 +223,30 @@ def main():
     ms_per_step = total_ms / args.steps
     value = world * 2.0 * updates / (ms_per_step * 1e-3) / 1e9
 
+    # ---- recon mode (row f2), reported beside the headline, never part of it -------------------------------
+    recon = None
+    if args.fbp:
+        q = torch.empty_like(y)
+        for _ in range(2):
+            geom.fbp_filter(y, views=sel, out=q)
+            geom.bp_recon(q, views=sel, out=xb)
+        barrier()
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps + 1)]
+        e[0].record(stream)
+        for i in range(args.steps):
+            geom.fbp_filter(y, views=sel, out=q)
+            e[2 * i + 1].record(stream)
+            geom.bp_recon(q, views=sel, out=xb)
+            e[2 * i + 2].record(stream)
+        barrier()
+        f_ms = float(np.mean([e[2 * i].elapsed_time(e[2 * i + 1]) for i in range(args.steps)]))
+        r_ms = float(np.mean([e[2 * i + 1].elapsed_time(e[2 * i + 2]) for i in range(args.steps)]))
+        taps = float(y.numel()) * c["nu"] / 2.0                      # fp64 multiply-adds of the ramp filter
+        recon = {"filter_ms": f_ms, "bp_recon_ms": r_ms, "bp_recon_gups": updates / (r_ms * 1e-3) / 1e9,
+                 "filter_fp64_tflops": 2.0 * taps / (f_ms * 1e-3) / 1e12,
+                 "fbp_gups": updates / ((f_ms + r_ms) * 1e-3) / 1e9}
+        del q
+
     # ---- end to end through the host-buffer entry points (pinned memory) -----------------------------
     e2e = None
     if not args.no_e2e:
@@ -271,7 +297,7 @@ def main():
                        "parallelism": "replicas" if world > 1 else "single"},
             "fp_ms": fp_ms, "bp_ms": bp_ms,
             "fp_gups": updates / (fp_ms * 1e-3) / 1e9, "bp_gups": updates / (bp_ms * 1e-3) / 1e9,
-            "gpu_launches": launches, "clocks": clocks, "e2e": e2e,
+            "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "recon": recon,
             "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": pk["fp32_tflops"],
                          "unit": "TFLOP/s", "frac": achieved / pk["fp32_tflops"], "traffic": traffic,
                          "peak_src": "148 SM x 128 fp32 lanes x 2 x %.0f MHz (MEASURED_PEAKS sm_max_mhz, %s)"

@@ -14,7 +14,8 @@
 
 namespace {
 
-constexpr int FLT_THREADS = 256;
+constexpr int FLT_THREADS = 128;
+constexpr int FJ = 8;              // outputs per thread (register tile of the Toeplitz product)
 
 template <int ARC>
 __global__ void __launch_bounds__(FLT_THREADS)
@@ -46,11 +47,46 @@ fbp_filter_kernel(SfProblem pr, const SfView *__restrict__ views, const float *_
         h[k] = hn;
     }
     __syncthreads();
+    // Each thread owns FJ outputs of one parity, k = kb + 2 j.  Only taps of the other parity contribute
+    // (h[even] = 0) besides the centre tap; for those m = m0 + 2 i the table index k - m drops by 2 per step, so
+    // the FJ table values in use form a sliding window: one new p'[m] and one new h per step feed FJ fp64 FMAs.
+    // The window lives in a register ring whose rotation is resolved at compile time by unrolling FJ steps.
     float *q = out + (size_t)row * pr.nu;
-    for (int k = tid; k < pr.nu; k += FLT_THREADS) {
-        double acc = pw[k] * h[0];
-        for (int m = (k + 1) & 1; m < pr.nu; m += 2) acc = fma(pw[m], h[abs(k - m)], acc);   // |k - m| odd only
-        q[k] = (float)(du * acc);
+    const int n_groups = (pr.nu + 2 * FJ - 1) / (2 * FJ);              // groups of FJ same-parity outputs
+    for (int gi = tid; gi < 2 * n_groups; gi += FLT_THREADS) {
+        const int par = gi & 1, kb = (gi >> 1) * (2 * FJ) + par;      // outputs kb, kb + 2, ...
+        const int m0 = 1 - par;                                        // taps m0, m0 + 2, ...
+        const int n_taps = (pr.nu - m0 + 1) / 2;
+        double acc[FJ], w[FJ];
+#pragma unroll
+        for (int j = 0; j < FJ; ++j) {
+            acc[j] = 0.0;
+            const int n = kb + 2 * j - m0;                             // table index of output j at step 0
+            w[j] = h[min(abs(n), pr.nu - 1)];
+        }
+        // ring: at step i the weight of output j sits in w[(j - i) mod FJ]
+        int i = 0;
+        for (; i + FJ <= n_taps; i += FJ) {
+#pragma unroll
+            for (int ii = 0; ii < FJ; ++ii) {
+                const double pm = pw[m0 + 2 * (i + ii)];
+#pragma unroll
+                for (int j = 0; j < FJ; ++j) acc[j] = fma(pm, w[(j - ii + FJ) % FJ], acc[j]);
+                // next step: output 0 needs h[|kb - m0 - 2 (i + ii + 1)|]; it replaces the slot output FJ-1 used
+                const int n = kb - m0 - 2 * (i + ii + 1);
+                w[(FJ - 1 - ii + FJ) % FJ] = h[min(abs(n), pr.nu - 1)];
+            }
+        }
+        for (; i < n_taps; ++i) {                                      // remainder: plain lookups
+            const double pm = pw[m0 + 2 * i];
+#pragma unroll
+            for (int j = 0; j < FJ; ++j) acc[j] = fma(pm, h[min(abs(kb + 2 * j - m0 - 2 * i), pr.nu - 1)], acc[j]);
+        }
+#pragma unroll
+        for (int j = 0; j < FJ; ++j) {
+            const int k = kb + 2 * j;
+            if (k < pr.nu) q[k] = (float)(du * fma(pw[k], h[0], acc[j]));
+        }
     }
 }
 
