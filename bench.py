@@ -281,7 +281,7 @@ def main():
         dom, dom_ms = ("ct_fp_sf", fp_ms) if fp_ms >= bp_ms else ("ct_bp_sf", bp_ms)
         traffic = None
         try:
-            traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(
+            traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.txt"))).get(
                 "config%d" % args.config, {}).get(dom)
         except Exception:
             pass
