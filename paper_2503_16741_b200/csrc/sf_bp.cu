@@ -99,8 +99,8 @@ bp_pixel_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
 // ---------------------------------------------------------------------------------------------------
 // 3-D: brick per CTA, detector tile in shared memory (TMA)
 // ---------------------------------------------------------------------------------------------------
-constexpr int BX = 16, BY = 16, BZ = 8;         // brick (voxels); 256 threads, one (x, y) column each
-constexpr int TW = 96, TH = 40;                  // detector tile (cells x rows) = one TMA box
+constexpr int BX = 16, BY = 16, BZ = 16;         // brick (voxels); 256 threads, one (x, y) column each
+constexpr int TW = 96, TH = 64;                  // detector tile (cells x rows) = one TMA box
 constexpr int LM = 4;                            // rows gathered per pass (registers f2[LM])
 constexpr int BRICK_THREADS = BX * BY;
 constexpr int TILE_FLOATS = TW * (TH + LM);      // + LM zero rows so row chunks never read outside
