@@ -15,6 +15,7 @@
 namespace {
 
 constexpr int FLT_THREADS = 128;
+__device__ __forceinline__ int HP(int n) { return n + (n >> 4); }   // padded table index
 constexpr int FJ = 8;              // outputs per thread (register tile of the Toeplitz product)
 
 template <int ARC>
@@ -23,7 +24,7 @@ fbp_filter_kernel(SfProblem pr, const SfView *__restrict__ views, const float *_
                   float *__restrict__ out, int view_begin, int view_stride, int view_count, double du, double dv)
 {
     extern __shared__ double sm[];
-    double *pw = sm, *h = sm + pr.nu;
+    double *pw = sm, *h = sm + pr.nu;             // h is stored padded: entry n at HP(n) = n + n/16
     const int tid = threadIdx.x;
     const long row = (long)blockIdx.x;                   // (batch * view_count + j) * nv + l
     const int l = (int)(row % pr.nv);
@@ -44,7 +45,7 @@ fbp_filter_kernel(SfProblem pr, const SfView *__restrict__ views, const float *_
         else if ((k & 1) == 0) hn = 0.0;
         else if (ARC == 0) { const double x = PI * k * du; hn = -1.0 / (x * x); }
         else { const double x = PI * R * sin(k * du / R); hn = -1.0 / (x * x); }
-        h[k] = hn;
+        h[k + (k >> 4)] = hn;
     }
     __syncthreads();
     // Each thread owns FJ outputs of one parity, k = kb + 2 j.  Only taps of the other parity contribute
@@ -53,8 +54,13 @@ fbp_filter_kernel(SfProblem pr, const SfView *__restrict__ views, const float *_
     // The window lives in a register ring whose rotation is resolved at compile time by unrolling FJ steps.
     float *q = out + (size_t)row * pr.nu;
     const int n_groups = (pr.nu + 2 * FJ - 1) / (2 * FJ);              // groups of FJ same-parity outputs
-    for (int gi = tid; gi < 2 * n_groups; gi += FLT_THREADS) {
-        const int par = gi & 1, kb = (gi >> 1) * (2 * FJ) + par;      // outputs kb, kb + 2, ...
+    // lane -> (parity, group): a half-warp holds 16 consecutive groups of one parity, whose table indices differ
+    // by 2 FJ = 16 -- with the table padded by one entry per 16 they fall into 16 different 8-byte banks
+    const int n_slots = ((n_groups + 15) / 16) * 32;
+    for (int gi = tid; gi < n_slots; gi += FLT_THREADS) {
+        const int par = (gi >> 4) & 1, grp = (gi >> 5) * 16 + (gi & 15);
+        if (grp >= n_groups) continue;
+        const int kb = grp * (2 * FJ) + par;                          // outputs kb, kb + 2, ...
         const int m0 = 1 - par;                                        // taps m0, m0 + 2, ...
         const int n_taps = (pr.nu - m0 + 1) / 2;
         double acc[FJ], w[FJ];
@@ -62,7 +68,7 @@ fbp_filter_kernel(SfProblem pr, const SfView *__restrict__ views, const float *_
         for (int j = 0; j < FJ; ++j) {
             acc[j] = 0.0;
             const int n = kb + 2 * j - m0;                             // table index of output j at step 0
-            w[j] = h[min(abs(n), pr.nu - 1)];
+            w[j] = h[HP(min(abs(n), pr.nu - 1))];
         }
         // ring: at step i the weight of output j sits in w[(j - i) mod FJ]
         int i = 0;
@@ -74,18 +80,18 @@ fbp_filter_kernel(SfProblem pr, const SfView *__restrict__ views, const float *_
                 for (int j = 0; j < FJ; ++j) acc[j] = fma(pm, w[(j - ii + FJ) % FJ], acc[j]);
                 // next step: output 0 needs h[|kb - m0 - 2 (i + ii + 1)|]; it replaces the slot output FJ-1 used
                 const int n = kb - m0 - 2 * (i + ii + 1);
-                w[(FJ - 1 - ii + FJ) % FJ] = h[min(abs(n), pr.nu - 1)];
+                w[(FJ - 1 - ii + FJ) % FJ] = h[HP(min(abs(n), pr.nu - 1))];
             }
         }
         for (; i < n_taps; ++i) {                                      // remainder: plain lookups
             const double pm = pw[m0 + 2 * i];
 #pragma unroll
-            for (int j = 0; j < FJ; ++j) acc[j] = fma(pm, h[min(abs(kb + 2 * j - m0 - 2 * i), pr.nu - 1)], acc[j]);
+            for (int j = 0; j < FJ; ++j) acc[j] = fma(pm, h[HP(min(abs(kb + 2 * j - m0 - 2 * i), pr.nu - 1))], acc[j]);
         }
 #pragma unroll
         for (int j = 0; j < FJ; ++j) {
             const int k = kb + 2 * j;
-            if (k < pr.nu) q[k] = (float)(du * fma(pw[k], h[0], acc[j]));
+            if (k < pr.nu) q[k] = (float)(du * fma(pw[k], h[0], acc[j]));      // HP(0) = 0
         }
     }
 }
@@ -98,7 +104,7 @@ int ctsf_launch_filter(const ct_geom *g, const float *d_proj, float *d_out, int 
     const SfProblem &pr = g->prob;
     const long rows = (long)batch * view_count * pr.nv;
     if (rows == 0) return 0;
-    const size_t smem = 2 * sizeof(double) * (size_t)pr.nu;
+    const size_t smem = sizeof(double) * (2 * (size_t)pr.nu + pr.nu / 16 + 2);
     if (smem > 200 * 1024) return -1;
     auto kern = pr.det_type ? fbp_filter_kernel<1> : fbp_filter_kernel<0>;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
