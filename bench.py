@@ -89,7 +89,7 @@ class ClockSampler:
         return out
 
 
-def cpu_baseline(c, x, budget_views=1, n_vox=32768):
+def cpu_baseline(c, x, budget_views=12, n_vox=1 << 20):
     """The oracle as it stands, on the host cores, on a bounded sample of the same workload."""
     from oracle.sf_oracle import Oracle
     o = Oracle(W.geom_keys(c))
@@ -124,7 +124,7 @@ def run_reference(args, c):
     times, cb = [], None
     for i in range(args.warmup + args.steps):
         t0 = time.perf_counter()
-        cb = cpu_baseline(c, x, budget_views=1, n_vox=8192)
+        cb = cpu_baseline(c, x, budget_views=2, n_vox=1 << 16)
         if i >= args.warmup:
             times.append(time.perf_counter() - t0)
     val = cb["value"]
