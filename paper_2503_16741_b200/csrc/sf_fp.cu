@@ -460,7 +460,11 @@ void launch_fp(const ct_geom *g, const float *d_vol, const float *d_volT, float 
     const size_t vbs = (size_t)pr.nx * pr.ny * pr.nz, pbs = (size_t)vc * pr.nv * pr.nu;
     constexpr int ROWS = DIM == 3 ? FTL + FLM : NB;
     const size_t smem = (size_t)FPW * ROWS * FTK * sizeof(float);
-    auto kern = (DIM == 3 && g->fp_hoist_ok && !getenv("CTSF_FP_NOHOIST")) ? fp_band_kernel<DIM, ARC, NB, DIM == 3 ? 1 : 0>
+    // testing aids: CTSF_FP_NOHOIST=1 never uses the untilted fast path; CTSF_FP_FORCEHOIST=1 uses it for every
+    // untilted 3-D geometry, also when footprints exceed its register windows (exercises its overflow branch)
+    const bool hoist = DIM == 3 && !getenv("CTSF_FP_NOHOIST") &&
+                       (g->fp_hoist_ok || (g->all_untilted && getenv("CTSF_FP_FORCEHOIST")));
+    auto kern = hoist ? fp_band_kernel<DIM, ARC, NB, DIM == 3 ? 1 : 0>
                                                                             : fp_band_kernel<DIM, ARC, NB, 0>;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const long n_items = (long)tiles_k * bands_l * ((vc + FPW - 1) / FPW) * FPW;

@@ -163,3 +163,34 @@ def test_config5_gradient_descent_against_oracle():
         assert abs(a - b) <= 1e-4 * abs(b), (losses_g, losses_o)
     _check(xg, xo, "x_10 of the config-5 loop", rel_tol=1e-4, max_tol=1e-3)
     geom.close()
+
+
+def test_untilted_fast_path_overflow_and_equivalence(monkeypatch):
+    """The forward kernel's untilted fast path keeps <= 6 footprint columns / <= 8 rows in registers and is only
+    chosen when the host's bound says that is enough.  Forced on geometries with larger footprints
+    (CTSF_FP_FORCEHOIST) its overflow branch must still give the oracle's answer; and on a geometry where both
+    paths apply, fast path and general path must agree to summation order."""
+    from paper_2503_16741_b200.projector import Geometry
+    for index, shrink in ((2, dict(nx=24, ny=22, nz=20, nu=320, nv=300, n_views=7)),     # K, L ~ 20
+                          (3, dict(nx=40, ny=36, nz=10, nu=400, nv=60, n_views=6))):     # arc, K ~ 10
+        c = W.make_config(index, **shrink)
+        g = W.geom_keys(c)
+        x = W.make_phantom(c)
+        o, geom = Oracle(g), Geometry(g)
+        monkeypatch.setenv("CTSF_FP_FORCEHOIST", "1")
+        y = geom.fp(torch.from_numpy(x).cuda())
+        torch.cuda.synchronize()
+        monkeypatch.delenv("CTSF_FP_FORCEHOIST")
+        _check(y, o.fp(x), "A forced fast path, config %d" % index)
+        geom.close()
+    c = W.make_config(2, nx=70, ny=66, nz=37, nu=150, nv=101, n_views=11)
+    geom = Geometry(W.geom_keys(c))
+    x = torch.from_numpy(W.make_phantom(c)).cuda()
+    y_fast = geom.fp(x)
+    torch.cuda.synchronize()
+    monkeypatch.setenv("CTSF_FP_NOHOIST", "1")
+    y_gen = geom.fp(x)
+    torch.cuda.synchronize()
+    monkeypatch.delenv("CTSF_FP_NOHOIST")
+    assert (y_fast - y_gen).abs().max().item() <= 3e-6 * y_gen.abs().max().item()
+    geom.close()
