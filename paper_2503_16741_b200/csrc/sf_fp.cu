@@ -105,7 +105,7 @@ __global__ void __launch_bounds__(32 * FPW, FMINB)
 fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ vol,
                const float *__restrict__ volT, float *__restrict__ proj, int view_begin, int view_stride,
                int tiles_k, int bands_l, int n_items, int n_views_sel, size_t vol_bstride, size_t proj_bstride,
-               float region_pad)
+               float region_pad, int force_serial)
 {
     constexpr int ROWS = DIM == 3 ? FTL + FLM : NB;
     extern __shared__ float smem[];
@@ -235,7 +235,7 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
                     const int j_b = livek ? min(k_hi, k_top) - k_lo : -1;
                     if (__reduce_max_sync(FULL, j_b + 1) == 0) continue;
                     const unsigned same = __match_any_sync(FULL, livek ? k_lo : INT_MIN + lane) & ~(1u << lane);
-                    const bool ok = __all_sync(FULL, same == 0u);
+                    const bool ok = __all_sync(FULL, same == 0u) && !force_serial;
                     float f1[FKR];                       // weight of column k_lo + j
                     {
                         float xi = (float)k_lo - T.kc, g0 = sf_G(T, xi);
@@ -389,7 +389,7 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
                 } else {
                     fine = same == 0u;
                 }
-                const bool ok = __all_sync(FULL, fine);
+                const bool ok = __all_sync(FULL, fine) && !force_serial;
                 const float amp = sf_amplitude(v, a, b, c, p, q);
 #pragma unroll
                 for (int bb = 0; bb < NB; ++bb) xv[bb] *= amp;
@@ -475,7 +475,8 @@ void launch_fp(const ct_geom *g, const float *d_vol, const float *d_volT, float 
     dim3 grid((unsigned)((n_items + FPW - 1) / FPW), groups, 1);
     kern<<<grid, 32 * FPW, smem, st>>>(pr, g->d_fp, d_vol + (size_t)b0 * vbs,
                                        d_volT ? d_volT + (size_t)b0 * vbs : nullptr,
-                                       d_proj + (size_t)b0 * pbs, vb, vs, tiles_k, bands_l, (int)n_items, vc, vbs, pbs, region_pad);
+                                       d_proj + (size_t)b0 * pbs, vb, vs, tiles_k, bands_l, (int)n_items, vc, vbs, pbs, region_pad,
+                                       getenv("CTSF_FP_SERIAL") ? 1 : 0);   // testing aid: take the lane-serial branch
 }
 
 template <int DIM, int ARC>

@@ -194,3 +194,22 @@ def test_untilted_fast_path_overflow_and_equivalence(monkeypatch):
     monkeypatch.delenv("CTSF_FP_NOHOIST")
     assert (y_fast - y_gen).abs().max().item() <= 3e-6 * y_gen.abs().max().item()
     geom.close()
+
+
+def test_forward_lane_serial_branch(monkeypatch):
+    """If a pass ever fails its conflict check the forward kernel adds the lanes' footprints one lane at a time.
+    The branch is never expected to run; forced (CTSF_FP_SERIAL) it must give the same answer."""
+    from paper_2503_16741_b200.projector import Geometry
+    for index, shrink in ((4, dict(nx=30, ny=28, nz=26, nu=70, nv=66, n_views=5)),
+                          (2, dict(nx=30, ny=28, nz=20, nu=64, nv=60, n_views=4)),
+                          (5, dict(nx=40, ny=36, nu=90, n_views=6, batch=2))):
+        c = W.make_config(index, **shrink)
+        g = W.geom_keys(c)
+        x = W.make_phantom(c)
+        o, geom = Oracle(g), Geometry(g)
+        monkeypatch.setenv("CTSF_FP_SERIAL", "1")
+        y = geom.fp(torch.from_numpy(x).cuda())
+        torch.cuda.synchronize()
+        monkeypatch.delenv("CTSF_FP_SERIAL")
+        _check(y, o.fp(x), "A lane-serial, config %d" % index)
+        geom.close()
