@@ -2,7 +2,7 @@
 //
 // Output-exclusive design, no atomics of any kind.  One WARP owns one detector tile of one view and
 // keeps it in shared memory for the whole pass.  It walks the voxel slabs perpendicular to the view's
-// dominant ray axis; per slab it inverse-projects the (expanded) tile onto the slab to find the voxels
+// dominant ray axis; per slab it inverse-projects the tile onto the slab to find the voxels
 // that can touch it, and adds their footprints into the tile in conflict-free "rounds" (see
 // fp_band_kernel).  Each detector cell is stored exactly once; the summation order is fixed.
 //
@@ -58,13 +58,15 @@ __device__ __forceinline__ Ray tile_ray(const SfView &v, float kf, float lf)
 // ---------------------------------------------------------------------------------------------------
 // One WARP owns one detector tile of one view: FTK cells x FTL rows (3-D) or FTK cells x NB images
 // (2-D), held in the warp's private slice of shared memory for the whole pass.  No block barrier is
-// ever executed.  Per slab the warp inverse-projects its (expanded) tile to a voxel rectangle and
-// sweeps it row by row: lane i takes voxel p = p_lo + i*sp (+ colour c < sp), computes its footprint
-// once, and the warp adds the footprints into the tile in K "rounds": in round j every lane updates
-// column k_lo(i) + j of its own footprint (all its rows).  k_lo is strictly monotone along the lanes
-// (sp is chosen on the host so that neighbouring lanes' voxels project >= 1 cell apart, and the
-// kernel verifies it with a warp match), so within a round the lanes touch pairwise different
-// columns; rounds are separated by __syncwarp().  Summation order is fixed => deterministic.
+// ever executed.  Per slab the warp inverse-projects its tile (rays through the tile corners + the exact
+// half-voxel halo) to the quadrilateral of voxels that can touch it and sweeps that region in sheared,
+// flattened order, 32 voxels per pass: lane i computes its voxel's footprint once, and the warp adds
+// the footprints into the tile in K "rounds": in round j every lane updates column k_lo(i) + j of its
+// own footprint (all its rows).  The lanes of a pass have pairwise different k_lo, or touch disjoint
+// rows (the host picks a lane stride so that neighbouring voxels project >= 1 cell apart; rows of equal
+// p are interleaved half a region apart; the kernel verifies both per pass with a warp match and
+// serialises the pass otherwise), so within a round no two lanes touch the same cell; rounds are
+// separated by __syncwarp().  Summation order is fixed => deterministic.
 constexpr int FPW = 8;            // warps per CTA
 constexpr int FMINB = 3;          // CTAs per SM the register budget is sized for
 constexpr int FTK = 64;           // cells per warp tile

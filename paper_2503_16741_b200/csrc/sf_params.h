@@ -34,7 +34,7 @@ struct SfView {
     float Up, Uq, Uz;
     float Vp, Vq, Vz;
     float ku0c, lv0c;          // detector coordinates (cells) of the point the Dm ray hits
-    float ek, el;              // tile expansion (cells / rows): max |footprint half extent| + margin
+    float ek, el;              // max footprint half extent (cells / rows) over the view, x1.1: host-side bound on K, L
     int32_t lane_stride;       // voxels p, p + lane_stride project >= 1 cell apart (conflict-free rounds)
     float recon_dR;            // recon mode (reading R23): d * R, d = distance source -> rotation centre (world origin)
     int32_t pad1, pad2;
