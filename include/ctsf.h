@@ -90,7 +90,8 @@ CTSF_API ct_status_t ct_bp_sf(const ct_geom_t *geom, const float *d_proj, float 
 
 /* Ordered-subset variants: the operators restricted to views
  * view_begin, view_begin + view_stride, ... (view_count of them).  The projection buffer holds
- * ONLY the selected views: [batch][view_count][nv][nu]. */
+ * ONLY the selected views: [batch][view_count][nv][nu].  view_count == 0 is the empty subset: the
+ * projection buffer has no elements (its pointer may be NULL), A writes nothing and A^T writes zeros. */
 CTSF_API ct_status_t ct_fp_sf_views(const ct_geom_t *geom, const float *d_vol, float *d_proj, int32_t batch,
                            int32_t view_begin, int32_t view_stride, int32_t view_count, ct_stream_t stream);
 CTSF_API ct_status_t ct_bp_sf_views(const ct_geom_t *geom, const float *d_proj, float *d_vol, int32_t batch,

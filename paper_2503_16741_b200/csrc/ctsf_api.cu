@@ -36,12 +36,28 @@ cudaMemPool_t pool_of_current_device()
     return g_pool[dev];
 }
 
-ct_status_t check_call(const ct_geom *g, const void *a, const void *b, int batch, int vb, int vs, int vc)
+// a = input, b = output.  With an empty view subset (vc == 0) the projection-side buffer has no elements and
+// may be NULL: `proj_is_a` tells which side that is.
+ct_status_t check_call(const ct_geom *g, const void *a, const void *b, int batch, int vb, int vs, int vc,
+                       bool proj_is_a = false, bool proj_is_b = false)
 {
-    if (!g || !a || !b || batch < 1) return CT_ERR_INVALID_ARG;
+    if (!g || batch < 1) return CT_ERR_INVALID_ARG;
+    if (vc == 0 && vs >= 1 && vb >= 0) {
+        if ((!a && !proj_is_a) || (!b && !proj_is_b)) return CT_ERR_INVALID_ARG;
+        return CT_OK;
+    }
+    if (!a || !b) return CT_ERR_INVALID_ARG;
     if (vc < 0 || vs < 1 || vb < 0) return CT_ERR_INVALID_ARG;
     if (vc > 0 && (long)vb + (long)(vc - 1) * vs >= g->prob.n_views) return CT_ERR_INVALID_ARG;
     if (((uintptr_t)a | (uintptr_t)b) & 15u) return CT_ERR_INVALID_ARG;
+    return CT_OK;
+}
+
+ct_status_t zero_volume(const ct_geom *g, float *d_vol, int batch, ct_stream_t stream)
+{
+    const size_t n = (size_t)batch * g->prob.nx * g->prob.ny * g->prob.nz;
+    if (cudaMemsetAsync(d_vol, 0, n * sizeof(float), (cudaStream_t)stream) != cudaSuccess) { cudaGetLastError(); return CT_ERR_CUDA; }
+    const_cast<ct_geom *>(g)->last_launches.store(0);
     return CT_OK;
 }
 
@@ -134,8 +150,9 @@ ct_status_t ct_geom_destroy(ct_geom_t *g)
 ct_status_t ct_fp_sf_views(const ct_geom_t *g, const float *d_vol, float *d_proj, int32_t batch,
                            int32_t vb, int32_t vs, int32_t vc, ct_stream_t stream)
 {
-    ct_status_t st = check_call(g, d_vol, d_proj, batch, vb, vs, vc);
+    ct_status_t st = check_call(g, d_vol, d_proj, batch, vb, vs, vc, false, true);
     if (st != CT_OK) return st;
+    if (vc == 0) { const_cast<ct_geom *>(g)->last_launches.store(0); return CT_OK; }     // nothing to write
     int n = ctsf_launch_fp(g, d_vol, d_proj, batch, vb, vs, vc, stream);
     if (n < 0) return CT_ERR_CUDA;
     const_cast<ct_geom *>(g)->last_launches.store(n);
@@ -145,8 +162,9 @@ ct_status_t ct_fp_sf_views(const ct_geom_t *g, const float *d_vol, float *d_proj
 ct_status_t ct_bp_sf_views(const ct_geom_t *g, const float *d_proj, float *d_vol, int32_t batch,
                            int32_t vb, int32_t vs, int32_t vc, ct_stream_t stream)
 {
-    ct_status_t st = check_call(g, d_proj, d_vol, batch, vb, vs, vc);
+    ct_status_t st = check_call(g, d_proj, d_vol, batch, vb, vs, vc, true, false);
     if (st != CT_OK) return st;
+    if (vc == 0) return zero_volume(g, d_vol, batch, stream);                            // empty sum
     int n = ctsf_launch_bp(g, d_proj, d_vol, batch, vb, vs, vc, stream);
     if (n < 0) return CT_ERR_CUDA;
     const_cast<ct_geom *>(g)->last_launches.store(n);
@@ -156,8 +174,9 @@ ct_status_t ct_bp_sf_views(const ct_geom_t *g, const float *d_proj, float *d_vol
 ct_status_t ct_bp_sf_recon_views(const ct_geom_t *g, const float *d_proj, float *d_vol, int32_t batch,
                                  int32_t vb, int32_t vs, int32_t vc, ct_stream_t stream)
 {
-    ct_status_t st = check_call(g, d_proj, d_vol, batch, vb, vs, vc);
+    ct_status_t st = check_call(g, d_proj, d_vol, batch, vb, vs, vc, true, false);
     if (st != CT_OK) return st;
+    if (vc == 0) return zero_volume(g, d_vol, batch, stream);
     int n = ctsf_launch_bp(g, d_proj, d_vol, batch, vb, vs, vc, stream, 0, 1);
     if (n < 0) return CT_ERR_CUDA;
     const_cast<ct_geom *>(g)->last_launches.store(n);
@@ -173,8 +192,9 @@ ct_status_t ct_bp_sf_recon(const ct_geom_t *g, const float *d_proj, float *d_vol
 ct_status_t ct_fbp_filter_views(const ct_geom_t *g, const float *d_proj, float *d_out, int32_t batch,
                                 int32_t vb, int32_t vs, int32_t vc, ct_stream_t stream)
 {
-    ct_status_t st = check_call(g, d_proj, d_out, batch, vb, vs, vc);
+    ct_status_t st = check_call(g, d_proj, d_out, batch, vb, vs, vc, true, true);
     if (st != CT_OK) return st;
+    if (vc == 0) { const_cast<ct_geom *>(g)->last_launches.store(0); return CT_OK; }
     if (d_proj == d_out) return CT_ERR_INVALID_ARG;           // not in place: every output reads the whole row
     int n = ctsf_launch_filter(g, d_proj, d_out, batch, vb, vs, vc, stream);
     if (n < 0) return CT_ERR_CUDA;

@@ -213,3 +213,20 @@ def test_forward_lane_serial_branch(monkeypatch):
         monkeypatch.delenv("CTSF_FP_SERIAL")
         _check(y, o.fp(x), "A lane-serial, config %d" % index)
         geom.close()
+
+
+def test_empty_view_subset():
+    """view_count == 0: A writes nothing (empty projection tensor), A^T is the empty sum (zeros)."""
+    from paper_2503_16741_b200.projector import Geometry
+    c = W.make_config(2, nx=20, ny=18, nz=12, nu=40, nv=30, n_views=6)
+    geom = Geometry(W.geom_keys(c))
+    x = torch.from_numpy(W.make_phantom(c)).cuda()
+    y = geom.fp(x, views=(2, 1, 0))
+    assert tuple(y.shape) == (1, 0, 30, 40)
+    xb = torch.full_like(x, float("nan"))
+    geom.bp(y, views=(2, 1, 0), out=xb)
+    assert torch.count_nonzero(xb).item() == 0
+    geom.bp_recon(y, views=(0, 1, 0), out=xb.fill_(float("nan")))
+    assert torch.count_nonzero(xb).item() == 0
+    assert tuple(geom.fbp_filter(y, views=(0, 1, 0)).shape) == (1, 0, 30, 40)
+    geom.close()
