@@ -206,7 +206,31 @@ __device__ __forceinline__ float gather_tile(const float *__restrict__ tile, con
     return sum;
 }
 
-template <int ARC, int RECON>
+// the same with the F1 weights of columns k_lo .. k_lo + K - 1 given (untilted frames, K <= BKR: computed once
+// per (x, y) column and view and reused along the z-run)
+constexpr int BKR = 6;
+__device__ __forceinline__ float gather_tile_w(const float *__restrict__ tile, const float (&f1)[BKR], int K,
+                                               const SfAxial &A, int k_lo, int l_lo, int l_hi, int tk0, int tl0)
+{
+    float sum = 0.0f;
+    for (int lb = l_lo; lb <= l_hi; lb += LM) {
+        float f2[LM];
+        sf_F2_run<LM>(A, (float)lb, f2);
+        const float *row = tile + (lb - tl0) * TW + (k_lo - tk0);
+#pragma unroll
+        for (int k = 0; k < BKR; ++k) {
+            if (k < K) {
+                float s = 0.0f;
+#pragma unroll
+                for (int j = 0; j < LM; ++j) s = fmaf(f2[j], row[j * TW + k], s);
+                sum = fmaf(f1[k], s, sum);
+            }
+        }
+    }
+    return sum;
+}
+
+template <int ARC, int RECON, int UNT>
 __global__ void __launch_bounds__(BRICK_THREADS, 3)
 bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ proj,
                 const __grid_constant__ CUtensorMap tmap, int use_tma, float *__restrict__ vol,
@@ -297,15 +321,27 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
                     }
                     if (col_in) {
                         // untilted frames: the transaxial footprint does not depend on z -> once per column
-                        const bool unt = v.untilted != 0;
+                        const bool unt = UNT || v.untilted != 0;
                         float a = a_col, b = b_col, inv_a = 0.0f;
                         SfTrans T;
                         int k_lo = 0, k_hi = -1;
+                        float f1[BKR], sumF1 = 0.0f;           // UNT: the weights themselves, once per column
                         if (unt) {
                             inv_a = rcp_nr(a);
                             sf_transaxial<ARC>(v, a, b, inv_a, T);
                             k_lo = max(max(0, tk0), (int)floorf(T.kc + T.t0));
                             k_hi = min(min(pr.nu - 1, tk0 + TW - 1), (int)floorf(T.kc + T.t3));
+                            if (UNT) {
+                                sumF1 = T.h01 + T.w12 + T.h23;
+                                float xi = (float)k_lo - T.kc, g0 = sf_G(T, xi);
+#pragma unroll
+                                for (int k = 0; k < BKR; ++k) {
+                                    xi += 1.0f;
+                                    const float g1 = sf_G(T, xi);
+                                    f1[k] = g1 - g0;
+                                    g0 = g1;
+                                }
+                            }
                         }
                         for (int zi = 0; zi <= z1 - z0; ++zi) {
                             const float z = (float)(z0 + zi);
@@ -323,9 +359,23 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
                             const int l_lo = max(max(0, tl0), (int)floorf(A.lc + A.tlo));
                             const int l_hi = min(min(pr.nv - 1, tl0 + TH - 1), (int)floorf(A.lc + A.thi));
                             if (l_lo > l_hi) continue;
-                            const float amp = RECON ? sf_recon_weight<ARC>(v, T, A.thi - A.tlo, a, b)
-                                                    : sf_amplitude(v, a, b, c, p, q);
-                            const float sum = gather_tile(tile, T, A, k_lo, k_hi, l_lo, l_hi, tk0, tl0);
+                            float amp, sum;
+                            if (UNT) {
+                                amp = RECON ? sf_recon_weight_s<ARC>(v, sumF1, A.thi - A.tlo, a, b)
+                                            : sf_amplitude(v, a, b, c, p, q);
+                                const int K = k_hi - k_lo + 1;
+                                if (K <= BKR) {
+                                    sum = gather_tile_w(tile, f1, K, A, k_lo, l_lo, l_hi, tk0, tl0);
+                                } else {            // footprint wider than the host's bound (never expected)
+                                    SfTrans T2;
+                                    sf_transaxial<ARC>(v, a, b, inv_a, T2);
+                                    sum = gather_tile(tile, T2, A, k_lo, k_hi, l_lo, l_hi, tk0, tl0);
+                                }
+                            } else {
+                                amp = RECON ? sf_recon_weight<ARC>(v, T, A.thi - A.tlo, a, b)
+                                            : sf_amplitude(v, a, b, c, p, q);
+                                sum = gather_tile(tile, T, A, k_lo, k_hi, l_lo, l_hi, tk0, tl0);
+                            }
                             float *ap = accs + zi * BRICK_THREADS + tid;
                             *ap = fmaf(amp, sum, *ap);
                         }
@@ -385,7 +435,12 @@ int launch_brick(const ct_geom *g, const float *d_proj, float *d_vol, int batch,
             use_tma = (dbg && dbg[0] >= '1' && dbg[0] <= '3') ? dbg[0] - '0' : 3;
     }
     const size_t smem = (size_t)(2 * TILE_FLOATS + BZ * BRICK_THREADS) * sizeof(float);
-    auto kern = recon ? bp_brick_kernel<ARC, 1> : bp_brick_kernel<ARC, 0>;
+    // untilted frames with small footprints (host bound): F1 weights live in registers along the z-run
+    // (testing aids: CTSF_BP_NOHOIST / CTSF_BP_FORCEHOIST, as for the forward kernel)
+    const bool hoist = !getenv("CTSF_BP_NOHOIST") &&
+                       (g->fp_hoist_ok || (g->all_untilted && getenv("CTSF_BP_FORCEHOIST")));
+    auto kern = hoist ? (recon ? bp_brick_kernel<ARC, 1, 1> : bp_brick_kernel<ARC, 0, 1>)
+                      : (recon ? bp_brick_kernel<ARC, 1, 0> : bp_brick_kernel<ARC, 0, 0>);
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const int nbz = (pr.nz + BZ - 1) / BZ;
     int launches = 0;

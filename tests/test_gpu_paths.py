@@ -178,10 +178,16 @@ def test_untilted_fast_path_overflow_and_equivalence(monkeypatch):
         x = W.make_phantom(c)
         o, geom = Oracle(g), Geometry(g)
         monkeypatch.setenv("CTSF_FP_FORCEHOIST", "1")
+        monkeypatch.setenv("CTSF_BP_FORCEHOIST", "1")
         y = geom.fp(torch.from_numpy(x).cuda())
+        y_ref = o.fp(x)
+        y32 = y_ref.astype(np.float32)
+        xb = geom.bp(torch.from_numpy(y32).cuda())
         torch.cuda.synchronize()
         monkeypatch.delenv("CTSF_FP_FORCEHOIST")
-        _check(y, o.fp(x), "A forced fast path, config %d" % index)
+        monkeypatch.delenv("CTSF_BP_FORCEHOIST")
+        _check(y, y_ref, "A forced fast path, config %d" % index)
+        _check(xb, o.bp(y32), "A^T forced fast path, config %d" % index)
         geom.close()
     c = W.make_config(2, nx=70, ny=66, nz=37, nu=150, nv=101, n_views=11)
     geom = Geometry(W.geom_keys(c))
@@ -193,6 +199,13 @@ def test_untilted_fast_path_overflow_and_equivalence(monkeypatch):
     torch.cuda.synchronize()
     monkeypatch.delenv("CTSF_FP_NOHOIST")
     assert (y_fast - y_gen).abs().max().item() <= 3e-6 * y_gen.abs().max().item()
+    xb_gen = geom.bp(y_gen)
+    torch.cuda.synchronize()
+    monkeypatch.setenv("CTSF_BP_NOHOIST", "1")
+    xb_gen2 = geom.bp(y_gen)
+    torch.cuda.synchronize()
+    monkeypatch.delenv("CTSF_BP_NOHOIST")
+    assert (xb_gen - xb_gen2).abs().max().item() <= 3e-6 * xb_gen2.abs().max().item()
     geom.close()
 
 
