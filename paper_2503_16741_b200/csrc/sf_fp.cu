@@ -211,6 +211,8 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
         const float q = (float)iq;
         const float aq0 = fmaf(q, v.aq, v.a0), bq0 = fmaf(q, v.bq, v.b0), cq0 = fmaf(q, v.cq, v.c0);
         const float *slab = src + (size_t)iq * np;
+        asm volatile("" : "+l"(slab));      // pin the slab pointer in registers (ptxas otherwise rebuilds it from the
+                                            // kernel parameters, ~14 instructions, in every pass)
 
         if (UNT) {
             // ---- untilted frames with small footprints (n.z = u.z = 0; K <= FKR columns, L <= 2 FLM rows) ---
