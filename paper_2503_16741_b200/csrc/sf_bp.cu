@@ -179,13 +179,42 @@ __device__ __forceinline__ TileInfo brick_shadow(const SfView &v, const SfProble
     return t;
 }
 
-// gather one voxel's footprint from the tile whose origin is (tk0, tl0); returns sum_kl F1 F2 y
-__device__ __forceinline__ float gather_tile(const float *__restrict__ tile, const SfTrans &T, const SfAxial &A,
+__device__ __forceinline__ float lds_f32(uint32_t a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
+
+// gather one voxel's footprint from the tile (shared-memory byte address tile_a) whose origin is (tk0, tl0);
+// returns sum_kl F1 F2 y.  The four row loads of a column are issued first (explicit ld.shared keeps that order),
+// the trapezoid CDF is evaluated under their latency.
+__device__ __forceinline__ float gather_tile(uint32_t tile_a, const SfTrans &T, const SfAxial &A,
                                              int k_lo, int k_hi, int l_lo, int l_hi, int tk0, int tl0)
 {
     float sum = 0.0f;
     for (int lb = l_lo; lb <= l_hi; lb += LM) {
         // rows past l_hi get weight 0 by themselves (x >= thi), rows past the tile read the zero pad rows
+        float f2[LM];
+        sf_F2_run<LM>(A, (float)lb, f2);
+        uint32_t ra = tile_a + 4u * (unsigned)((lb - tl0) * TW + (k_lo - tk0));
+        float xi = (float)k_lo - T.kc;
+        float g0 = sf_G(T, xi);
+#pragma unroll 1
+        for (int k = k_lo; k <= k_hi; ++k, ra += 4) {
+            const float y0 = lds_f32(ra), y1 = lds_f32(ra + 4 * TW), y2 = lds_f32(ra + 8 * TW), y3 = lds_f32(ra + 12 * TW);
+            xi += 1.0f;
+            const float g1 = sf_G(T, xi);
+            float s = f2[0] * y0;
+            s = fmaf(f2[1], y1, s); s = fmaf(f2[2], y2, s); s = fmaf(f2[3], y3, s);
+            sum = fmaf(g1 - g0, s, sum);
+            g0 = g1;
+        }
+    }
+    return sum;
+}
+
+// plain-pointer version (compiler-scheduled loads): the overflow branch of the untilted kernels
+__device__ __forceinline__ float gather_tile_ptr(const float *__restrict__ tile, const SfTrans &T, const SfAxial &A,
+                                                 int k_lo, int k_hi, int l_lo, int l_hi, int tk0, int tl0)
+{
+    float sum = 0.0f;
+    for (int lb = l_lo; lb <= l_hi; lb += LM) {
         float f2[LM];
         sf_F2_run<LM>(A, (float)lb, f2);
         const float *row = tile + (lb - tl0) * TW + (k_lo - tk0);
@@ -305,6 +334,8 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
         if (t.live) {
             const SfView v = sview[s];          // local copy: the fields in use stay in registers over the z-run
             float *tile = s ? tile1 : tile0;
+            uint32_t tile_a = smem_u32(tile);
+            if (!UNT) asm volatile("" : "+r"(tile_a));   // one register instead of a rebuild per voxel
             const float a_col = fmaf(q, v.aq, fmaf(p, v.ap, v.a0));
             const float b_col = fmaf(q, v.bq, fmaf(p, v.bp, v.b0));
             const float c_col = fmaf(q, v.cq, fmaf(p, v.cp, v.c0));
@@ -369,12 +400,12 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
                                 } else {            // footprint wider than the host's bound (never expected)
                                     SfTrans T2;
                                     sf_transaxial<ARC>(v, a, b, inv_a, T2);
-                                    sum = gather_tile(tile, T2, A, k_lo, k_hi, l_lo, l_hi, tk0, tl0);
+                                    sum = gather_tile_ptr(tile, T2, A, k_lo, k_hi, l_lo, l_hi, tk0, tl0);
                                 }
                             } else {
                                 amp = RECON ? sf_recon_weight<ARC>(v, T, A.thi - A.tlo, a, b)
                                             : sf_amplitude(v, a, b, c, p, q);
-                                sum = gather_tile(tile, T, A, k_lo, k_hi, l_lo, l_hi, tk0, tl0);
+                                sum = gather_tile(tile_a, T, A, k_lo, k_hi, l_lo, l_hi, tk0, tl0);
                             }
                             float *ap = accs + zi * BRICK_THREADS + tid;
                             *ap = fmaf(amp, sum, *ap);
