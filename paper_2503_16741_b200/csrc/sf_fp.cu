@@ -68,6 +68,7 @@ __device__ __forceinline__ Ray tile_ray(const SfView &v, float kf, float lf)
 // serialises the pass otherwise), so within a round no two lanes touch the same cell; rounds are
 // separated by __syncwarp().  Summation order is fixed => deterministic.
 constexpr int FPW = 8;            // warps per CTA
+constexpr int FVG = 48;           // views per item group (multiple of FPW): consecutive CTAs sweep one tile of FVG views
 constexpr int FMINB = 3;          // CTAs per SM the register budget is sized for
 constexpr int FTK = 64;           // cells per warp tile
 constexpr int FTL = 32;           // rows per warp tile (3-D)
@@ -116,12 +117,13 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int item = blockIdx.x * FPW + warp;
     if (item >= n_items) return;                     // warps are independent: no block barrier below
-    // item order: groups of FPW consecutive views; within a group tile-major, view fastest -- the
-    // warps of one CTA sweep the SAME tile of FPW neighbouring views, whose frusta nearly coincide,
-    // so the volume is pulled through L1/L2 once per group of views instead of once per view
+    // item order: groups of FVG consecutive views; within a group tile-major, view fastest -- the
+    // warps of one CTA (and the next FVG/FPW - 1 CTAs) sweep the SAME tile of neighbouring views, whose
+    // frusta nearly coincide, so the volume is pulled through L1/L2 once per group of views instead of
+    // once per view
     const int per_view = tiles_k * bands_l;
-    const int grp = item / (per_view * FPW), rem_g = item - grp * (per_view * FPW);
-    const int rem = rem_g / FPW, jview = grp * FPW + (rem_g - rem * FPW);
+    const int grp = item / (per_view * FVG), rem_g = item - grp * (per_view * FVG);
+    const int rem = rem_g / FVG, jview = grp * FVG + (rem_g - rem * FVG);
     if (jview >= n_views_sel) return;
     const int bl = rem / tiles_k, tk = rem - bl * tiles_k;
     const int k0 = tk * FTK, l0 = bl * FTL;
@@ -471,7 +473,7 @@ void launch_fp(const ct_geom *g, const float *d_vol, const float *d_volT, float 
     auto kern = hoist ? fp_band_kernel<DIM, ARC, NB, DIM == 3 ? 1 : 0>
                                                                             : fp_band_kernel<DIM, ARC, NB, 0>;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    const long n_items = (long)tiles_k * bands_l * ((vc + FPW - 1) / FPW) * FPW;
+    const long n_items = (long)tiles_k * bands_l * ((vc + FVG - 1) / FVG) * FVG;
     // testing aid: CTSF_FP_PAD=<voxels> widens the swept voxel region; the result must not change beyond
     // summation order (tests/test_gpu_fullsize.py uses it to prove that the tight region misses nothing)
     const char *pad_env = getenv("CTSF_FP_PAD");
