@@ -14,7 +14,7 @@ from paper_2503_16741_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
 
-N_VIEWS = {1: 6, 2: 3, 3: 3, 4: 2, 5: 4}
+N_VIEWS = {1: 6, 2: 5, 3: 5, 4: 6, 5: 4}
 N_VOX = {1: 4000, 2: 3000, 3: 3000, 4: 3000, 5: 3000}
 
 
