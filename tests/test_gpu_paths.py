@@ -243,3 +243,26 @@ def test_empty_view_subset():
     assert torch.count_nonzero(xb).item() == 0
     assert tuple(geom.fbp_filter(y, views=(0, 1, 0)).shape) == (1, 0, 30, 40)
     geom.close()
+
+
+@pytest.mark.parametrize("env", [{"CTSF_BP_TMA": "0"}, {"CTSF_BP_CHUNK": "3"}, {"CTSF_BP_TMA": "0", "CTSF_BP_CHUNK": "5"}])
+def test_backprojector_alternate_staging_and_chunking(env, monkeypatch):
+    """The backprojector with cp.async tile staging instead of TMA, and with its view loop cut into many small
+    launches (accumulating), must give the same answer as the default configuration and as the oracle."""
+    from paper_2503_16741_b200.projector import Geometry
+    c = W.make_config(4, nx=44, ny=48, nz=40, nu=112, nv=100, n_views=17)
+    g = W.geom_keys(c)
+    o, geom = Oracle(g), Geometry(g)
+    y32 = o.fp(W.make_phantom(c)).astype(np.float32)
+    yd = torch.from_numpy(y32).cuda()
+    x_default = geom.bp(yd)
+    torch.cuda.synchronize()
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    x_alt = geom.bp(yd)
+    torch.cuda.synchronize()
+    for k in env:
+        monkeypatch.delenv(k)
+    _check(x_alt, o.bp(y32), "A^T with %s" % env)
+    assert (x_alt - x_default).abs().max().item() <= 3e-6 * x_default.abs().max().item()
+    geom.close()
