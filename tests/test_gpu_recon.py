@@ -75,3 +75,26 @@ def test_fbp_of_an_analytic_ball_on_the_gpu():
     mid = 0.5 * (x[c["nz"] // 2 - 1] + x[c["nz"] // 2])
     assert abs(mid[inside].mean() / mu - 1.0) < 1e-2, mid[inside].mean() / mu
     geom.close()
+
+
+def test_curved_detector_with_lateral_offset_all_operators():
+    """PAPER.md:151 scenario (curved detector, 1.25-channel lateral offset) through the CTorch-style converter
+    with clockwise view angles: A, A^T, the ramp filter and the recon backprojection against the oracle."""
+    from paper_2503_16741_b200 import geometry as G
+    from paper_2503_16741_b200.projector import Geometry
+    n_views, nu, du = 31, 230, 1.2
+    g = G.Geom2D(nx=100, ny=94, dx=0.5, dy=0.5, nu=nu, du=du, nView=n_views,
+                 viewAngles=-np.linspace(0.0, 2.0 * math.pi, n_views, endpoint=False), detType="curved",
+                 SAD=595.0, SDD=1085.6, uOfst=1.25 * du)
+    c = W.make_config(5, nx=100, ny=94, nu=nu, n_views=n_views, batch=2)     # phantom recipe only
+    x = W.make_phantom(c)
+    o, geom = Oracle(g), Geometry(g)
+    y_ref = o.fp(x)
+    _check(geom.fp(torch.from_numpy(x).cuda()), y_ref, "A offset arc")
+    y32 = y_ref.astype(np.float32)
+    _check(geom.bp(torch.from_numpy(y32).cuda()), o.bp(y32), "A^T offset arc")
+    q_ref = o.fbp_filter(y32)
+    _check(geom.fbp_filter(torch.from_numpy(y32).cuda()), q_ref, "filter offset arc")
+    q32 = q_ref.astype(np.float32)
+    _check(geom.bp_recon(torch.from_numpy(q32).cuda()), o.bp_recon(q32), "recon BP offset arc")
+    geom.close()

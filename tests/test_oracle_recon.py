@@ -107,3 +107,23 @@ def test_recon_backprojection_weights_are_normalised():
         a = np.dot(P - c["src"][i], n)
         want += np.dot(-c["src"][i], n) * R / a ** 2
     assert abs(x[iz, iy, ix] / want - 1.0) < 1e-12
+
+
+def test_fbp_curved_detector_with_lateral_offset():
+    """curved detector "with a 1.25-pixel lateral offset" (there: AAPM CT-MAR sinograms; here an
+    analytic disk).  Geometry through the CTorch-style converter (PAPER.md:114-116 conventions, clockwise view
+    angles as in the paper's listing); the offset must not bias the reconstruction."""
+    from paper_2503_16741_b200 import geometry as G
+    n_views, nu, du = 240, 220, 1.2
+    g = G.Geom2D(nx=96, ny=96, dx=0.5, dy=0.5, nu=nu, du=du, nView=n_views,
+                 viewAngles=-np.linspace(0.0, 2.0 * math.pi, n_views, endpoint=False), detType="curved",
+                 SAD=595.0, SDD=1085.6, uOfst=1.25 * du)
+    c = dict(g, n_views=n_views)
+    centre, radius = (4.0, -3.0, 0.0), 10.0
+    x = _fbp(c, _ball_projections(c, radius, centre))[0]
+    xs = (np.arange(96) - 47.5) * 0.5
+    X, Y = np.meshgrid(xs, xs)
+    r = np.hypot(X - centre[0], Y - centre[1])
+    inside = r < 0.8 * radius
+    assert abs(x[inside].mean() / MU - 1.0) < 5e-3, x[inside].mean() / MU
+    assert np.abs(x[inside] / MU - 1.0).max() < 3e-2
