@@ -266,3 +266,21 @@ def test_backprojector_alternate_staging_and_chunking(env, monkeypatch):
     _check(x_alt, o.bp(y32), "A^T with %s" % env)
     assert (x_alt - x_default).abs().max().item() <= 3e-6 * x_default.abs().max().item()
     geom.close()
+
+
+def test_backward_direction_module_gradient_is_forward_projection():
+    """"forward projection and backprojection are gradients of each other".  For the module in
+    direction 'backward' (x = A^T y) autograd's gradient of <w, A^T y> with respect to y must be A w."""
+    from paper_2503_16741_b200.projector import Projector
+    c = W.make_config(2, nx=24, ny=22, nz=16, nu=48, nv=40, n_views=6)
+    At = Projector(W.geom_keys(c), "proj", "SF", "backward")
+    rng = np.random.default_rng(3)
+    y = torch.from_numpy(rng.uniform(0, 1, (1, 6, 40, 48)).astype(np.float32)).cuda().requires_grad_()
+    w = torch.from_numpy(rng.uniform(0, 1, (1, 16, 22, 24)).astype(np.float32)).cuda()
+    loss = (At(y) * w).sum()
+    (grad,) = torch.autograd.grad(loss, [y])
+    want = At.geom.fp(w)
+    assert torch.allclose(grad, want, rtol=1e-6, atol=1e-6 * want.abs().max().item())
+    # ordered subsets through the module
+    sub = At(y[:, 1::2].contiguous(), subset=(1, 2, 3))
+    assert torch.equal(sub, At.geom.bp(y.detach()[:, 1::2].contiguous(), views=(1, 2, 3)))
