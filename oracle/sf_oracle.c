@@ -41,6 +41,7 @@ typedef struct {
     const double *det_center;/* [n_views][3] */
     const double *det_u;     /* [n_views][3] */
     const double *det_v;     /* [n_views][3]; dim 2: ignored, taken as (0,0,1) */
+    int model;               /* 0: separable footprint SF-TR; 1: distance-driven DD (row f4, reading R26) */
 } sfo_geom;
 
 /* O1: per-view frame. */
@@ -120,6 +121,23 @@ static int footprint(const sfo_geom *g, const sfo_frame *f, int ix, int iy, int 
             if (!det_coords(g, f, P, &tau[c], &t_unused)) return 0;       /* O2 */
             ++c;
         }
+    if (g->model == 1) {
+        /* R26, distance-driven (DD considers a "face-based voxel model"): the voxel is its
+         * central face perpendicular to the axis the voxel-centre ray mostly runs along.  The face's two
+         * in-plane edges -- (x_c +- dx/2, y_c) when the ray runs mostly along y, i.e. dy/|e_y| <= dx/|e_x|,
+         * else (x_c, y_c +- dy/2) -- project to s_a <= s_b and the transaxial footprint is the RECTANGLE on
+         * [s_a, s_b] (a trapezoid with zero-width ramps); the axial one stays the rectangle of O5 (the
+         * face's two z edges); the amplitude O6 is the slab thickness along the ray, as for SF. */
+        double ex = fabs(Pc[0] - f->S[0]), ey = fabs(Pc[1] - f->S[1]);
+        int along_y = g->dy * ex <= g->dx * ey;                    /* dy/|e_y| <= dx/|e_x| */
+        double Pa[3] = { Pc[0], Pc[1], Pc[2] }, Pb[3] = { Pc[0], Pc[1], Pc[2] };
+        if (along_y) { Pa[0] -= 0.5*g->dx; Pb[0] += 0.5*g->dx; } else { Pa[1] -= 0.5*g->dy; Pb[1] += 0.5*g->dy; }
+        double sa, sb, t_unused;
+        if (!det_coords(g, f, Pa, &sa, &t_unused)) return 0;
+        if (!det_coords(g, f, Pb, &sb, &t_unused)) return 0;
+        tau[0] = tau[1] = sa < sb ? sa : sb;
+        tau[2] = tau[3] = sa < sb ? sb : sa;
+    }
     sort4(tau);
     if (tau_out) memcpy(tau_out, tau, sizeof tau);
     /* O4: transaxial cell range and cell-averaged weights (R3, R12, R15) */

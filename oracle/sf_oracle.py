@@ -33,7 +33,7 @@ class _Geom(ctypes.Structure):
                 ("du", ctypes.c_double), ("dv", ctypes.c_double),
                 ("det_type", ctypes.c_int), ("n_views", ctypes.c_int),
                 ("src", ctypes.c_void_p), ("det_center", ctypes.c_void_p),
-                ("det_u", ctypes.c_void_p), ("det_v", ctypes.c_void_p)]
+                ("det_u", ctypes.c_void_p), ("det_v", ctypes.c_void_p), ("model", ctypes.c_int)]
 
 
 _lib = None
@@ -67,7 +67,7 @@ def _f64(a):
 class Oracle:
     """One scan geometry.  `g` is a plain dict with the keys of the problem description:
     dim, nx, ny, nz, dx, dy, dz, ox, oy, oz, nu, nv, du, dv, det_type ('flat'|'arc' or 0|1),
-    src, det_center, det_u, det_v (each [n_views, 3], float64)."""
+    src, det_center, det_u, det_v (each [n_views, 3], float64); optional algo 'SF' (default) | 'DD'."""
 
     def __init__(self, g):
         self.lib = _load()
@@ -90,7 +90,8 @@ class Oracle:
                        self.nu, self.nv, float(g["du"]), float(g.get("dv", 1.0)),
                        int(det), self.n_views,
                        self.src.ctypes.data, self.dc.ctypes.data,
-                       self.du_vec.ctypes.data, self.dv_vec.ctypes.data)
+                       self.du_vec.ctypes.data, self.dv_vec.ctypes.data,
+                       {"SF": 0, "DD": 1}.get(g.get("algo", "SF"), g.get("algo", 0)))
         self.threads = 0
 
     # -- pins ------------------------------------------------------------------------------
