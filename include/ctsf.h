@@ -66,7 +66,13 @@ typedef struct {
     const double *det_u;         /* HOST [n_views][3] unit vector along channels */
     const double *det_v;         /* HOST [n_views][3] unit vector along rows (arc: the cylinder axis);
                                     may be NULL when dim==2 (taken as (0,0,1)) */
+    int32_t algo;                /* voxel model of every operator of this geometry:
+                                    CT_ALGO_SF = 0 separable footprint, trapezoid x rectangle ("volume-based");
+                                    CT_ALGO_DD = 1 distance-driven ("face-based": the voxel's central face
+                                    perpendicular to the ray's dominant axis, rectangle x rectangle; R26) */
 } ct_geom_desc_t;
+
+enum { CT_ALGO_SF = 0, CT_ALGO_DD = 1 };
 
 /* Validates `desc`, derives the per-view kernel parameters in float64, rounds them to fp32 and
  * uploads them to the current CUDA device.  The host arrays are copied; the caller may free them

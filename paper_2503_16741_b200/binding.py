@@ -34,7 +34,7 @@ class ct_geom_desc_t(ctypes.Structure):
                 ("du", ctypes.c_double), ("dv", ctypes.c_double),
                 ("det_type", ctypes.c_int32), ("n_views", ctypes.c_int32),
                 ("src", ctypes.c_void_p), ("det_center", ctypes.c_void_p),
-                ("det_u", ctypes.c_void_p), ("det_v", ctypes.c_void_p)]
+                ("det_u", ctypes.c_void_p), ("det_v", ctypes.c_void_p), ("algo", ctypes.c_int32)]
 
 
 _lib = None
@@ -82,7 +82,7 @@ def _check(status, what):
 
 def ct_geom_create(g):
     """g: dict with the ct_geom_desc_t keys (det_type 'flat'|'arc' or 0|1; vectors as [n_views,3]
-    float64 arrays).  Returns an opaque handle (int) for the calls below."""
+    float64 arrays; optional algo 'SF' (default) | 'DD').  Returns an opaque handle (int) for the calls below."""
     src = np.ascontiguousarray(g["src"], dtype=np.float64).reshape(-1, 3)
     dc = np.ascontiguousarray(g["det_center"], dtype=np.float64).reshape(-1, 3)
     du = np.ascontiguousarray(g["det_u"], dtype=np.float64).reshape(-1, 3)
@@ -97,7 +97,8 @@ def ct_geom_create(g):
                        float(g.get("ox", 0.0)), float(g.get("oy", 0.0)), float(g.get("oz", 0.0)),
                        int(g["nu"]), int(g.get("nv", 1)), float(g["du"]), float(g.get("dv", 1.0)),
                        int(det), int(n_views), src.ctypes.data, dc.ctypes.data, du.ctypes.data,
-                       None if dv is None else dv.ctypes.data)
+                       None if dv is None else dv.ctypes.data,
+                       int({"SF": 0, "DD": 1}.get(g.get("algo", "SF"), g.get("algo", 0))))
     out = ctypes.c_void_p()
     _check(lib().ct_geom_create(ctypes.byref(d), ctypes.byref(out)), "ct_geom_create")
     return out.value

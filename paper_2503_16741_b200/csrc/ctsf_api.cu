@@ -91,6 +91,7 @@ ct_status_t ct_geom_create(const ct_geom_desc_t *d, ct_geom_t **out)
     if (d->dim == 3 && (!finite_pos(d->dz) || !finite_pos(d->dv))) return CT_ERR_INVALID_ARG;
     if (!std::isfinite(d->ox) || !std::isfinite(d->oy) || (d->dim == 3 && !std::isfinite(d->oz))) return CT_ERR_INVALID_ARG;
     if (d->det_type != 0 && d->det_type != 1) return CT_ERR_INVALID_ARG;
+    if (d->algo != CT_ALGO_SF && d->algo != CT_ALGO_DD) return CT_ERR_INVALID_ARG;
     if (!d->src || !d->det_center || !d->det_u || (d->dim == 3 && !d->det_v)) return CT_ERR_INVALID_ARG;
     if ((double)d->nx * d->ny * d->nz >= 2147483648.0 || (double)d->nu * d->nv * d->n_views >= 2147483648.0 * 4)
         return CT_ERR_UNSUPPORTED;
@@ -103,6 +104,7 @@ ct_status_t ct_geom_create(const ct_geom_desc_t *d, ct_geom_t **out)
     if (!g) return CT_ERR_ALLOC;
     g->prob = SfProblem{d->dim, d->det_type, d->nx, d->ny, d->nz, d->nu, d->nv, d->n_views};
     g->du = d->du;
+    g->model = d->algo;
     g->dv = d->dim == 3 ? d->dv : 1.0;
     ct_status_t st;
     try {

@@ -9,6 +9,7 @@
 struct ct_geom {
     SfProblem prob;
     double du = 1.0, dv = 1.0;        // detector pitches, mm (ramp filter)
+    int model = 0;                    // 0 separable footprint (SF-TR), 1 distance-driven (DD)
     std::vector<SfView> h_bp, h_fp;   // host copies (natural order / forward order with xy swaps)
     SfView *d_bp = nullptr, *d_fp = nullptr;
     int any_swap = 0;                 // some forward view reads the volume through its transpose

@@ -29,7 +29,7 @@ namespace {
 // ---------------------------------------------------------------------------------------------------
 constexpr int BP_VC = 16;     // views staged per chunk
 
-template <int ARC, int NB, int RECON>
+template <int ARC, int NB, int RECON, int MODEL>
 __global__ void __launch_bounds__(128)
 bp_pixel_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ proj,
                 float *__restrict__ vol, int view_begin, int view_stride, int view_count,
@@ -68,7 +68,7 @@ bp_pixel_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
             const float b = fmaf(q, v.bq, fmaf(p, v.bp, v.b0));
             const float inv_a = rcp_nr(a);
             SfTrans T;
-            sf_transaxial<ARC>(v, a, b, inv_a, T);
+            sf_transaxial<ARC, MODEL>(v, a, b, inv_a, T, p, q);
             const int k_lo = max(0, (int)floorf(T.kc + T.t0));
             const int k_hi = min(pr.nu - 1, (int)floorf(T.kc + T.t3));
             if (k_lo > k_hi) continue;
@@ -77,9 +77,9 @@ bp_pixel_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
             float sum[NB];
 #pragma unroll
             for (int bb = 0; bb < NB; ++bb) sum[bb] = 0.0f;
-            float g0 = sf_G(T, (float)k_lo - T.kc);
+            float g0 = sf_G<MODEL>(T, (float)k_lo - T.kc);
             for (int k = k_lo; k <= k_hi; ++k) {
-                const float g1 = sf_G(T, (float)(k + 1) - T.kc);
+                const float g1 = sf_G<MODEL>(T, (float)(k + 1) - T.kc);
                 const float f1 = g1 - g0;
                 g0 = g1;
 #pragma unroll
@@ -184,6 +184,7 @@ __device__ __forceinline__ float lds_f32(uint32_t a) { float v; asm volatile("ld
 // gather one voxel's footprint from the tile (shared-memory byte address tile_a) whose origin is (tk0, tl0);
 // returns sum_kl F1 F2 y.  The four row loads of a column are issued first (explicit ld.shared keeps that order),
 // the trapezoid CDF is evaluated under their latency.
+template <int MODEL>
 __device__ __forceinline__ float gather_tile(uint32_t tile_a, const SfTrans &T, const SfAxial &A,
                                              int k_lo, int k_hi, int l_lo, int l_hi, int tk0, int tl0)
 {
@@ -194,12 +195,12 @@ __device__ __forceinline__ float gather_tile(uint32_t tile_a, const SfTrans &T, 
         sf_F2_run<LM>(A, (float)lb, f2);
         uint32_t ra = tile_a + 4u * (unsigned)((lb - tl0) * TW + (k_lo - tk0));
         float xi = (float)k_lo - T.kc;
-        float g0 = sf_G(T, xi);
+        float g0 = sf_G<MODEL>(T, xi);
 #pragma unroll 1
         for (int k = k_lo; k <= k_hi; ++k, ra += 4) {
             const float y0 = lds_f32(ra), y1 = lds_f32(ra + 4 * TW), y2 = lds_f32(ra + 8 * TW), y3 = lds_f32(ra + 12 * TW);
             xi += 1.0f;
-            const float g1 = sf_G(T, xi);
+            const float g1 = sf_G<MODEL>(T, xi);
             float s = f2[0] * y0;
             s = fmaf(f2[1], y1, s); s = fmaf(f2[2], y2, s); s = fmaf(f2[3], y3, s);
             sum = fmaf(g1 - g0, s, sum);
@@ -210,6 +211,7 @@ __device__ __forceinline__ float gather_tile(uint32_t tile_a, const SfTrans &T, 
 }
 
 // plain-pointer version (compiler-scheduled loads): the overflow branch of the untilted kernels
+template <int MODEL>
 __device__ __forceinline__ float gather_tile_ptr(const float *__restrict__ tile, const SfTrans &T, const SfAxial &A,
                                                  int k_lo, int k_hi, int l_lo, int l_hi, int tk0, int tl0)
 {
@@ -219,11 +221,11 @@ __device__ __forceinline__ float gather_tile_ptr(const float *__restrict__ tile,
         sf_F2_run<LM>(A, (float)lb, f2);
         const float *row = tile + (lb - tl0) * TW + (k_lo - tk0);
         float xi = (float)k_lo - T.kc;
-        float g0 = sf_G(T, xi);
+        float g0 = sf_G<MODEL>(T, xi);
 #pragma unroll 1
         for (int k = k_lo; k <= k_hi; ++k) {
             xi += 1.0f;
-            const float g1 = sf_G(T, xi);
+            const float g1 = sf_G<MODEL>(T, xi);
             float s = 0.0f;
 #pragma unroll
             for (int j = 0; j < LM; ++j) s = fmaf(f2[j], row[j * TW], s);
@@ -259,7 +261,7 @@ __device__ __forceinline__ float gather_tile_w(const float *__restrict__ tile, c
     return sum;
 }
 
-template <int ARC, int RECON, int UNT>
+template <int ARC, int RECON, int UNT, int MODEL>
 __global__ void __launch_bounds__(BRICK_THREADS, 3)
 bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ proj,
                 const __grid_constant__ CUtensorMap tmap, int use_tma, float *__restrict__ vol,
@@ -359,16 +361,16 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
                         float f1[BKR], sumF1 = 0.0f;           // UNT: the weights themselves, once per column
                         if (unt) {
                             inv_a = rcp_nr(a);
-                            sf_transaxial<ARC>(v, a, b, inv_a, T);
+                            sf_transaxial<ARC, MODEL>(v, a, b, inv_a, T, p, q);
                             k_lo = max(max(0, tk0), (int)floorf(T.kc + T.t0));
                             k_hi = min(min(pr.nu - 1, tk0 + TW - 1), (int)floorf(T.kc + T.t3));
                             if (UNT) {
                                 sumF1 = T.h01 + T.w12 + T.h23;
-                                float xi = (float)k_lo - T.kc, g0 = sf_G(T, xi);
+                                float xi = (float)k_lo - T.kc, g0 = sf_G<MODEL>(T, xi);
 #pragma unroll
                                 for (int k = 0; k < BKR; ++k) {
                                     xi += 1.0f;
-                                    const float g1 = sf_G(T, xi);
+                                    const float g1 = sf_G<MODEL>(T, xi);
                                     f1[k] = g1 - g0;
                                     g0 = g1;
                                 }
@@ -379,7 +381,7 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
                             if (!unt) {
                                 a = fmaf(z, v.az, a_col); b = fmaf(z, v.bz, b_col);
                                 inv_a = rcp_nr(a);
-                                sf_transaxial<ARC>(v, a, b, inv_a, T);
+                                sf_transaxial<ARC, MODEL>(v, a, b, inv_a, T, p, q);
                                 k_lo = max(max(0, tk0), (int)floorf(T.kc + T.t0));
                                 k_hi = min(min(pr.nu - 1, tk0 + TW - 1), (int)floorf(T.kc + T.t3));
                             }
@@ -399,13 +401,13 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
                                     sum = gather_tile_w(tile, f1, K, A, k_lo, l_lo, l_hi, tk0, tl0);
                                 } else {            // footprint wider than the host's bound (never expected)
                                     SfTrans T2;
-                                    sf_transaxial<ARC>(v, a, b, inv_a, T2);
-                                    sum = gather_tile_ptr(tile, T2, A, k_lo, k_hi, l_lo, l_hi, tk0, tl0);
+                                    sf_transaxial<ARC, MODEL>(v, a, b, inv_a, T2, p, q);
+                                    sum = gather_tile_ptr<MODEL>(tile, T2, A, k_lo, k_hi, l_lo, l_hi, tk0, tl0);
                                 }
                             } else {
                                 amp = RECON ? sf_recon_weight<ARC>(v, T, A.thi - A.tlo, a, b)
                                             : sf_amplitude(v, a, b, c, p, q);
-                                sum = gather_tile(tile_a, T, A, k_lo, k_hi, l_lo, l_hi, tk0, tl0);
+                                sum = gather_tile<MODEL>(tile_a, T, A, k_lo, k_hi, l_lo, l_hi, tk0, tl0);
                             }
                             float *ap = accs + zi * BRICK_THREADS + tid;
                             *ap = fmaf(amp, sum, *ap);
@@ -470,8 +472,11 @@ int launch_brick(const ct_geom *g, const float *d_proj, float *d_vol, int batch,
     // (testing aids: CTSF_BP_NOHOIST / CTSF_BP_FORCEHOIST, as for the forward kernel)
     const bool hoist = !getenv("CTSF_BP_NOHOIST") &&
                        (g->fp_hoist_ok || (g->all_untilted && getenv("CTSF_BP_FORCEHOIST")));
-    auto kern = hoist ? (recon ? bp_brick_kernel<ARC, 1, 1> : bp_brick_kernel<ARC, 0, 1>)
-                      : (recon ? bp_brick_kernel<ARC, 1, 0> : bp_brick_kernel<ARC, 0, 0>);
+    auto kern = g->model == 1
+        ? (hoist ? (recon ? bp_brick_kernel<ARC, 1, 1, 1> : bp_brick_kernel<ARC, 0, 1, 1>)
+                 : (recon ? bp_brick_kernel<ARC, 1, 0, 1> : bp_brick_kernel<ARC, 0, 0, 1>))
+        : (hoist ? (recon ? bp_brick_kernel<ARC, 1, 1, 0> : bp_brick_kernel<ARC, 0, 1, 0>)
+                 : (recon ? bp_brick_kernel<ARC, 1, 0, 0> : bp_brick_kernel<ARC, 0, 0, 0>));
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const int nbz = (pr.nz + BZ - 1) / BZ;
     int launches = 0;
@@ -509,7 +514,8 @@ void launch_pixel(const ct_geom *g, const float *d_proj, float *d_vol, int b0, i
     const size_t pbs = (size_t)vc * pr.nu, vbs = (size_t)pr.nx * pr.ny;
     dim3 block(16, 8, 1);
     dim3 grid((pr.nx + block.x - 1) / block.x, (pr.ny + block.y - 1) / block.y, groups);
-    auto kern = recon ? bp_pixel_kernel<ARC, NB, 1> : bp_pixel_kernel<ARC, NB, 0>;
+    auto kern = g->model == 1 ? (recon ? bp_pixel_kernel<ARC, NB, 1, 1> : bp_pixel_kernel<ARC, NB, 0, 1>)
+                              : (recon ? bp_pixel_kernel<ARC, NB, 1, 0> : bp_pixel_kernel<ARC, NB, 0, 0>);
     kern<<<grid, block, 0, st>>>(pr, g->d_bp, d_proj + (size_t)b0 * pbs, d_vol + (size_t)b0 * vbs,
                                  vb, vs, vc, (unsigned)pbs, (unsigned)vbs);
 }

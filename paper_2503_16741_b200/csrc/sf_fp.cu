@@ -103,7 +103,7 @@ __device__ __forceinline__ void fp_round_rows(uint32_t ca, float w, const float 
     }
 }
 
-template <int DIM, int ARC, int NB, int UNT>
+template <int DIM, int ARC, int NB, int UNT, int MODEL>
 __global__ void __launch_bounds__(32 * FPW, FMINB)
 fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ vol,
                const float *__restrict__ volT, float *__restrict__ proj, int view_begin, int view_stride,
@@ -233,7 +233,7 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
                     const float a = fmaf(p, v_ap, aq0), b = fmaf(p, v_bp, bq0), cpq = fmaf(p, v_cp, cq0);
                     const float inv_a = rcp_nr(a);
                     SfTrans T;
-                    sf_transaxial<ARC>(v, a, b, inv_a, T);
+                    sf_transaxial<ARC, MODEL>(v, a, b, inv_a, T, p, q);
                     const int k_lo = (int)floorf(T.kc + T.t0);
                     const int k_hi = (int)floorf(T.kc + T.t3);
                     const bool livek = actp && k_hi >= k0 && k_lo <= k_top;
@@ -244,11 +244,11 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
                     const bool ok = __all_sync(FULL, same == 0u) && !force_serial;
                     float f1[FKR];                       // weight of column k_lo + j
                     {
-                        float xi = (float)k_lo - T.kc, g0 = sf_G(T, xi);
+                        float xi = (float)k_lo - T.kc, g0 = sf_G<MODEL>(T, xi);
 #pragma unroll
                         for (int j = 0; j < FKR; ++j) {
                             xi += 1.0f;
-                            const float g1 = sf_G(T, xi);
+                            const float g1 = sf_G<MODEL>(T, xi);
                             f1[j] = g1 - g0;
                             g0 = g1;
                         }
@@ -310,11 +310,11 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
                                     float g2[2 * FLM];
                                     sf_F2_run<2 * FLM>(A, (float)(l_lo + lb), g2);
                                     SfTrans T2;                  // recomputed here so that T need not stay live
-                                    sf_transaxial<ARC>(v, a, b, inv_a, T2);
+                                    sf_transaxial<ARC, MODEL>(v, a, b, inv_a, T2, p, q);
                                     for (int jk = (lb == 0 ? FKR : 0); jk < Kall; ++jk) {
                                         if (mine && jk >= j_a && jk <= j_b) {
                                             const float xi = (float)(k_lo + jk) - T2.kc;
-                                            const float w = (sf_G(T2, xi + 1.0f) - sf_G(T2, xi)) * ax;
+                                            const float w = (sf_G<MODEL>(T2, xi + 1.0f) - sf_G<MODEL>(T2, xi)) * ax;
                                             fp_round_rows<false, true>(ca + 4u * jk + 4u * FTK * lb, w, g2, L - lb);
                                         }
                                         __syncwarp();
@@ -371,7 +371,7 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
                     if (!__any_sync(FULL, act && l_lo <= l_hi)) continue;
                 }
                 SfTrans T;
-                sf_transaxial<ARC>(v, a, b, inv_a, T);
+                sf_transaxial<ARC, MODEL>(v, a, b, inv_a, T, p, q);
                 // unclipped column range: rounds are aligned on it, columns off the tile are skipped
                 const int k_lo = (int)floorf(T.kc + T.t0);
                 const int k_hi = (int)floorf(T.kc + T.t3);
@@ -410,14 +410,14 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
                             if (Lmax > lb + FLM) sf_F2_run<2 * FLM>(A, (float)(l_lo + lb), f2);
                             else                 sf_F2_run<FLM>(A, (float)(l_lo + lb), f2);
                         }
-                        float xi = xi0, g0 = sf_G(T, xi0);
+                        float xi = xi0, g0 = sf_G<MODEL>(T, xi0);
                         uint32_t ca = smem_addr(base + lb * FTK);      // this lane's cell of round 0
                         const int nrow = L - lb;
 #define CTSF_ROUNDS(...)                                             \
                         for (int jk = 0; jk < Kmax; ++jk, ca += 4) {   \
                             if (jk >= j_a && jk <= jb) {               \
                                 xi += 1.0f;                            \
-                                const float g1 = sf_G(T, xi);          \
+                                const float g1 = sf_G<MODEL>(T, xi);          \
                                 const float f1 = g1 - g0;              \
                                 g0 = g1;                               \
                                 __VA_ARGS__                            \
@@ -470,8 +470,9 @@ void launch_fp(const ct_geom *g, const float *d_vol, const float *d_volT, float 
     // untilted 3-D geometry, also when footprints exceed its register windows (exercises its overflow branch)
     const bool hoist = DIM == 3 && !getenv("CTSF_FP_NOHOIST") &&
                        (g->fp_hoist_ok || (g->all_untilted && getenv("CTSF_FP_FORCEHOIST")));
-    auto kern = hoist ? fp_band_kernel<DIM, ARC, NB, DIM == 3 ? 1 : 0>
-                                                                            : fp_band_kernel<DIM, ARC, NB, 0>;
+    auto kern = g->model == 1
+        ? (hoist ? fp_band_kernel<DIM, ARC, NB, DIM == 3 ? 1 : 0, 1> : fp_band_kernel<DIM, ARC, NB, 0, 1>)
+        : (hoist ? fp_band_kernel<DIM, ARC, NB, DIM == 3 ? 1 : 0, 0> : fp_band_kernel<DIM, ARC, NB, 0, 0>);
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const long n_items = (long)tiles_k * bands_l * ((vc + FVG - 1) / FVG) * FVG;
     // testing aid: CTSF_FP_PAD=<voxels> widens the swept voxel region; the result must not change beyond

@@ -18,6 +18,7 @@ class Geometry:
         torch.cuda.current_device()          # make sure a context exists before libctsf allocates
         torch.zeros(1, device="cuda")
         self.handle = B.ct_geom_create(g)
+        self.algo = {0: "SF", 1: "DD"}.get(g.get("algo", "SF"), g.get("algo", "SF"))
         self.dim = int(g["dim"])
         self.vol_shape = (int(g.get("nz", 1)), int(g["ny"]), int(g["nx"]))
         self.n_views = len(g["src"])
@@ -135,20 +136,25 @@ class BP(torch.autograd.Function):
 
 class Projector(torch.nn.Module):
     """`A = Projector(geom, 'proj', 'SF', 'forward'); sino = A(img)` (PAPER.md:118-122).
-    Algorithm 'SF' only; mode 'proj' (matched pair, differentiable) or 'recon' (FBP backprojection of
+    Algorithm 'SF' (separable footprint) or 'DD' (distance-driven); mode 'proj' (matched pair, differentiable) or 'recon' (FBP backprojection of
     PAPER.md:103, direction 'backward' only); direction is 'forward' or 'backward'.
     `subset=(view_begin, view_stride, view_count)` restricts to an ordered subset."""
 
     def __init__(self, geom, mode="proj", algo="SF", direction="forward"):
         super().__init__()
-        if mode not in ("proj", "recon") or algo != "SF":
-            raise NotImplementedError("only algo='SF' with mode 'proj' or 'recon' is built (see DESIGN.md)")
+        if mode not in ("proj", "recon") or algo not in ("SF", "DD"):
+            raise NotImplementedError("algo 'SF' or 'DD' with mode 'proj' or 'recon' is built (see DESIGN.md)")
         if direction not in ("forward", "backward"):
             raise ValueError(direction)
         if mode == "recon" and direction != "backward":
             raise NotImplementedError("'recon' mode is the FBP backprojection: direction must be 'backward'")
         self.mode = mode
-        self.geom = geom if isinstance(geom, Geometry) else Geometry(geom)
+        if isinstance(geom, Geometry):
+            if geom.algo != algo:
+                raise ValueError("the Geometry was created for algo=%r, not %r" % (geom.algo, algo))
+            self.geom = geom
+        else:
+            self.geom = Geometry(dict(geom, algo=algo))
         self.direction = direction
 
     def forward(self, x, subset=None):

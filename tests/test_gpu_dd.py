@@ -1,0 +1,75 @@
+"""GPU parity for the distance-driven model (reading R26): the same kernels with the
+rectangle x rectangle footprint of the voxel's central face, against the float64 oracle (algo='DD').
+Tolerances as for SF: rel-L2 <= 1e-5, max-abs <= 1e-4 max|oracle|, adjoint 1e-5."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle.sf_oracle import Oracle
+from paper_2503_16741_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+SHRINK = {
+    1: dict(nx=77, ny=70, nu=300, n_views=19),
+    2: dict(nx=70, ny=66, nz=37, nu=150, nv=101, n_views=11),
+    3: dict(nx=90, ny=84, nz=19, nu=301, nv=40, n_views=13),
+    4: dict(nx=61, ny=64, nz=58, nu=140, nv=135, n_views=12),
+    5: dict(nx=96, ny=90, nu=290, n_views=17, batch=5),
+}
+
+
+def _check(gpu, ref, what):
+    gpu = gpu.double().cpu().numpy()
+    rel = np.linalg.norm(gpu - ref) / np.linalg.norm(ref)
+    mx = np.abs(gpu - ref).max() / np.abs(ref).max()
+    assert rel <= 1e-5 and mx <= 1e-4, "%s: rel-L2 %.3e max-abs/max %.3e" % (what, rel, mx)
+
+
+@pytest.mark.parametrize("index", [1, 2, 3, 4, 5])
+def test_dd_parity_small(index):
+    from paper_2503_16741_b200.projector import Geometry
+    c = W.make_config(index, **SHRINK[index])
+    g = dict(W.geom_keys(c), algo="DD")
+    x = W.make_phantom(c)
+    o, geom = Oracle(g), Geometry(g)
+    y_ref = o.fp(x)
+    y = geom.fp(torch.from_numpy(x).cuda())
+    _check(y, y_ref, "DD A config %d" % index)
+    assert np.abs(y_ref - Oracle(W.geom_keys(c)).fp(x)).max() > 1e-3 * np.abs(y_ref).max()   # not SF's answer
+    y32 = y_ref.astype(np.float32)
+    _check(geom.bp(torch.from_numpy(y32).cuda()), o.bp(y32), "DD A^T config %d" % index)
+    rng = np.random.default_rng(200 + index)
+    xr = torch.from_numpy(rng.uniform(0, 1, x.shape).astype(np.float32)).cuda()
+    yr = torch.from_numpy(rng.uniform(0, 1, y_ref.shape).astype(np.float32)).cuda()
+    lhs = torch.sum(geom.fp(xr).double() * yr.double()).item()
+    rhs = torch.sum(xr.double() * geom.bp(yr).double()).item()
+    assert abs(lhs - rhs) <= 1e-5 * abs(lhs), (lhs, rhs)
+    # recon mode with the DD footprint
+    q32 = o.fbp_filter(y32).astype(np.float32)
+    _check(geom.bp_recon(torch.from_numpy(q32).cuda()), o.bp_recon(q32), "DD recon A^T config %d" % index)
+    geom.close()
+
+
+def test_dd_full_size_config4_sampled():
+    from paper_2503_16741_b200.projector import Geometry, Projector
+    c = W.make_config(4)
+    g = dict(W.geom_keys(c), algo="DD")
+    o = Oracle(g)
+    rng = np.random.default_rng(99)
+    x = W.make_phantom(c)
+    A = Projector(W.geom_keys(c), "proj", "DD", "forward")
+    y = A.geom.fp(torch.from_numpy(x).cuda())
+    views = np.sort(rng.choice(c["n_views"], 3, replace=False))
+    y_ref = o.fp(x, views)
+    _check(y[:, torch.from_numpy(views).cuda()], y_ref, "DD A config 4 full size")
+    del y
+    p = W.make_projections(c)
+    xb = A.geom.bp(torch.from_numpy(p).cuda())
+    ijk = np.stack([rng.integers(0, c["nx"], 2000), rng.integers(0, c["ny"], 2000), rng.integers(0, c["nz"], 2000)], axis=1)
+    ref = o.bp_voxels(p[0], ijk)
+    got = xb[0, ijk[:, 2], ijk[:, 1], ijk[:, 0]].double().cpu().numpy()
+    assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= 1e-5
+    assert np.abs(got - ref).max() <= 1e-4 * np.abs(ref).max()
+    A.geom.close()
