@@ -153,6 +153,8 @@ def main():
     ap.add_argument("--impl", default="ctsf")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--algo", default="SF", choices=["SF", "DD"],
+                    help="voxel model: SF (separable footprint, the headline) or DD (distance-driven, row f4)")
     ap.add_argument("--fbp", action="store_true",
                     help="also time recon mode (row f2): ct_fbp_filter + ct_bp_sf_recon on the step's projections")
     ap.add_argument("--view-stride", type=int, default=1,
@@ -176,7 +178,7 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    g = W.geom_keys(c)
+    g = dict(W.geom_keys(c), algo=args.algo)
     x_host = W.make_phantom(c)                         # [B, nz, ny, nx] fp32, seeded
     batch = c["batch"]
     geom = Geometry(g)
@@ -297,7 +299,7 @@ def main():
             "metric": metric_name(args.config), "value": value, "unit": "GUPS", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": c["name"], "index": args.config, "volume": [c["nz"], c["ny"], c["nx"]],
+            "config": {"workload": c["name"], "algo": args.algo, "index": args.config, "volume": [c["nz"], c["ny"], c["nx"]],
                        "views": n_sel, "detector": [c["nv"], c["nu"]], "batch": batch,
                        "step": "1 x ct_fp_sf + 1 x ct_bp_sf", "updates_per_operator": updates,
                        "l2": "inputs (%.0f MB) exceed the 126 MB L2; no flush" % (alg_bytes / 1e6),

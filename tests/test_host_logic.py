@@ -66,6 +66,13 @@ def test_descriptor_validation_without_gpu():
         assert status() in (4, 5)
 
 
+def test_unknown_algo_is_refused():
+    c = W.make_config(1, nx=8, ny=8, nu=16, n_views=3)
+    with pytest.raises(B.CtError) as e:
+        B.ct_geom_create(dict(W.geom_keys(c), algo=7))
+    assert e.value.status == 1
+
+
 def test_converter_identities():
     n = 16
     th = 2 * np.pi * np.arange(n) / n
