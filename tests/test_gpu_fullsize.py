@@ -59,8 +59,9 @@ def test_parity_full_size_sampled(index):
     geom.close()
 
 
+@pytest.mark.parametrize("algo", ["SF", "DD"])
 @pytest.mark.parametrize("index", [4, 3, 2])
-def test_forward_region_is_conservative(index, monkeypatch):
+def test_forward_region_is_conservative(index, algo, monkeypatch):
     """The forward kernel sweeps, per slab, only the voxels its tile's frustum can touch (exact half-voxel halo).
     Property that holds at any size: widening that region by a whole voxel (CTSF_FP_PAD) may only change the
     summation order.  Checked on EVERY cell of every view of the full-size operator (a missed voxel would
@@ -69,7 +70,7 @@ def test_forward_region_is_conservative(index, monkeypatch):
     c = W.make_config(index)
     if index == 4:
         c = W.make_config(index, n_views=96)          # every 7.5th view of the trajectory, full volume/detector
-    g = W.geom_keys(c)
+    g = dict(W.geom_keys(c), algo=algo)
     rng = np.random.default_rng(77 + index)
     x = torch.from_numpy(rng.uniform(0.5, 1.5, (1, c["nz"], c["ny"], c["nx"])).astype(np.float32)).cuda()
     geom = Geometry(g)
@@ -85,13 +86,14 @@ def test_forward_region_is_conservative(index, monkeypatch):
     geom.close()
 
 
+@pytest.mark.parametrize("algo", ["SF", "DD"])
 @pytest.mark.parametrize("index", [2, 5])
-def test_run_to_run_determinism(index):
+def test_run_to_run_determinism(index, algo):
     """Both operators fix their summation order (no atomics; the forward kernel's conflict-free rounds), so
     repeated calls are bit-identical.  A shared-memory race in the forward tile would show up here."""
     from paper_2503_16741_b200.projector import Geometry
     c = W.make_config(index)
-    g = W.geom_keys(c)
+    g = dict(W.geom_keys(c), algo=algo)
     rng = np.random.default_rng(5 + index)
     x = torch.from_numpy(rng.uniform(0, 1, (c["batch"], c["nz"], c["ny"], c["nx"])).astype(np.float32)).cuda()
     geom = Geometry(g)
