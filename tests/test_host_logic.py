@@ -201,3 +201,13 @@ def test_bench_reference_arm_under_torchrun_world2():
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["unit"] == "GUPS" and d["value"] > 0
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["value"] == d["value"]
+
+
+def test_header_is_plain_c(tmp_path):
+    """include/ctsf.h is the boundary: it must compile as C (no C++ or CUDA types) and as C++."""
+    import subprocess
+    src = tmp_path / "use.c"
+    src.write_text('#include "ctsf.h"\nint main(void) { ct_geom_desc_t d; (void)d; return (int)sizeof(ct_geom_desc_t) == 0; }\n')
+    inc = os.path.join(ROOT, "include")
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-pedantic", "-fsyntax-only", "-I", inc, str(src)])
+    subprocess.check_call(["g++", "-std=c++17", "-Wall", "-Werror", "-fsyntax-only", "-x", "c++", "-I", inc, str(src)])
