@@ -39,24 +39,33 @@ class _Geom(ctypes.Structure):
 _lib = None
 
 
+def _declare(lib):
+    lib.sfo_trap_cdf.restype = ctypes.c_double
+    lib.sfo_trap_cdf.argtypes = [ctypes.c_void_p, ctypes.c_double]
+    lib.sfo_live_fraction.restype = ctypes.c_double
+    P, I = ctypes.c_void_p, ctypes.c_int
+    lib.sfo_live_fraction.argtypes = [P, I, I]
+    lib.sfo_footprint.argtypes = [P, I, I, I, I, P, P, P, P, P]
+    lib.sfo_det_coords.argtypes = [P, I, P, P]
+    lib.sfo_fp.argtypes = [P, P, P, I, P]
+    lib.sfo_bp.argtypes = [P, P, P, I, P]
+    lib.sfo_fbp_filter.argtypes = [P, P, P, I, P]
+    lib.sfo_bp_recon.argtypes = [P, P, P, I, P]
+    lib.sfo_bp_voxels.argtypes = [P, P, P, I, P]
+    lib.sfo_bp_voxels_f32.argtypes = [P, P, P, I, P]
+    return lib
+
+
+def load_library(path):
+    """A build of sf_oracle.c other than the in-tree one (tests/test_oracle_mutations.py loads deliberately
+    broken copies through this to prove that the pins notice)."""
+    return _declare(ctypes.CDLL(path))
+
+
 def _load():
     global _lib
     if _lib is None:
-        lib = ctypes.CDLL(build())
-        lib.sfo_trap_cdf.restype = ctypes.c_double
-        lib.sfo_trap_cdf.argtypes = [ctypes.c_void_p, ctypes.c_double]
-        lib.sfo_live_fraction.restype = ctypes.c_double
-        P, I = ctypes.c_void_p, ctypes.c_int
-        lib.sfo_live_fraction.argtypes = [P, I, I]
-        lib.sfo_footprint.argtypes = [P, I, I, I, I, P, P, P, P, P]
-        lib.sfo_det_coords.argtypes = [P, I, P, P]
-        lib.sfo_fp.argtypes = [P, P, P, I, P]
-        lib.sfo_bp.argtypes = [P, P, P, I, P]
-        lib.sfo_fbp_filter.argtypes = [P, P, P, I, P]
-        lib.sfo_bp_recon.argtypes = [P, P, P, I, P]
-        lib.sfo_bp_voxels.argtypes = [P, P, P, I, P]
-        lib.sfo_bp_voxels_f32.argtypes = [P, P, P, I, P]
-        _lib = lib
+        _lib = _declare(ctypes.CDLL(build()))
     return _lib
 
 
