@@ -17,7 +17,7 @@ STATUS_NAMES = {0: "CT_OK", 1: "CT_ERR_INVALID_ARG", 2: "CT_ERR_GEOMETRY", 3: "C
                 4: "CT_ERR_ALLOC", 5: "CT_ERR_CUDA"}
 EXPORTS = ("ct_geom_create", "ct_geom_destroy", "ct_fp_sf", "ct_bp_sf", "ct_fp_sf_views", "ct_bp_sf_views",
            "ct_fp_sf_host", "ct_bp_sf_host", "ct_fbp_filter", "ct_fbp_filter_views", "ct_bp_sf_recon",
-           "ct_bp_sf_recon_views", "ct_last_launch_count", "ct_status_string")
+           "ct_bp_sf_recon_views", "ct_measure_fp32_peak", "ct_last_launch_count", "ct_status_string")
 
 
 class CtError(RuntimeError):
@@ -61,11 +61,12 @@ def lib():
         L.ct_bp_sf_recon.argtypes = [P, P, P, I, P]
         L.ct_fbp_filter_views.argtypes = [P, P, P, I, I, I, I, P]
         L.ct_bp_sf_recon_views.argtypes = [P, P, P, I, I, I, I, P]
+        L.ct_measure_fp32_peak.argtypes = [I, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), P]
         L.ct_last_launch_count.argtypes = [P]
         L.ct_last_launch_count.restype = I
         L.ct_status_string.argtypes = [ctypes.c_int]
         L.ct_status_string.restype = ctypes.c_char_p
-        for name in EXPORTS[:12]:
+        for name in EXPORTS[:13]:
             getattr(L, name).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -152,6 +153,14 @@ def ct_fbp_filter(handle, d_proj, d_out, batch, stream=0):
 
 def ct_bp_sf_recon(handle, d_proj, d_vol, batch, stream=0):
     _check(lib().ct_bp_sf_recon(handle, d_proj, d_vol, batch, stream), "ct_bp_sf_recon")
+
+
+def ct_measure_fp32_peak(kind=0, stream=0):
+    """Measured fp32 FMA throughput of the current device: (flop/s, seconds of the timed launch).
+    kind 0: scalar FFMA, 1: packed FFMA2."""
+    f, t = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _check(lib().ct_measure_fp32_peak(int(kind), ctypes.byref(f), ctypes.byref(t), stream), "ct_measure_fp32_peak")
+    return f.value, t.value
 
 
 def ct_last_launch_count(handle):

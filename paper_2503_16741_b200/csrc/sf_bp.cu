@@ -103,6 +103,9 @@ constexpr int BX = 16, BY = 16, BZ = 16;         // brick (voxels); 256 threads,
 constexpr int TW = 96, TH = 64;                  // detector tile (cells x rows) = one TMA box
 constexpr int LM = 4;                            // rows gathered per pass (registers f2[LM])
 constexpr int BRICK_THREADS = BX * BY;
+#ifndef BP2_MINB
+#define BP2_MINB 2                               // CTAs per SM the packed kernel's register budget is sized for
+#endif
 constexpr int TILE_FLOATS = TW * (TH + LM);      // + LM zero rows so row chunks never read outside
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -427,6 +430,215 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
     }
 }
 
+// ---------------------------------------------------------------------------------------------------
+// General (tilted-frame) brick kernel, two voxels per thread, barrier-free view pipeline.
+// Same brick / shadow / TMA-tile scheme as bp_brick_kernel, but
+//  (1) every thread walks its z-run in PAIRS (z, z + 1) and evaluates both footprints in lockstep with the packed
+//      FFMA2 / FMUL2 / FADD2 instructions of sm_100 (sf_footprint.cuh, "Packed pairs"): the kernel is bound by
+//      instruction issue, and the packed forms carry two voxels' multiply-adds in one issue slot.  The column and
+//      row loops run over max(K_a, K_b) x max(L_a, L_b); each footprint is cut at its own last cell edges, so the
+//      cells past them weigh exactly 0 (their loads stay inside the CTA's shared memory);
+//  (2) the views flow through a ring of BP2_STAGES tile buffers guarded by mbarrier pairs: full[s] completes when
+//      the TMA bytes of the view have landed (warp 0 stages the view's parameters and the brick's shadow and arms
+//      it), empty[s] when all warps have finished reading the stage.  No __syncthreads in the view loop: warps
+//      drift up to a view apart instead of waiting for the slowest one at every view (0.9 barrier stalls per
+//      issued instruction in the round-1 kernel).  Shadows larger than one box (rare) fall back to block-wide
+//      cp.async staging inside the view, which re-synchronises the CTA.
+// Accumulators: one float2 per thread and z-pair in shared memory, thread-private and conflict-free (a register
+// array indexed by the z loop would force the loop to be fully unrolled: 8 copies of the ~600-instruction body).
+// Requires the TMA path (16-byte aligned pitch and base); otherwise the launcher takes bp_brick_kernel.
+#ifndef BP2_STAGES_N
+#define BP2_STAGES_N 3
+#endif
+#ifndef BP2_SERIES
+#define BP2_SERIES 0
+#endif
+constexpr int BP2_STAGES = BP2_STAGES_N;
+
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+template <int ARC, int RECON, int MODEL>
+__global__ void __launch_bounds__(BRICK_THREADS, BP2_MINB)
+bp_brick2_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ proj,
+                 const __grid_constant__ CUtensorMap tmap, float *__restrict__ vol,
+                 int view_begin, int view_stride, int view_count, int j_lo, int j_hi, int nbz, int accumulate)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float *tiles = reinterpret_cast<float *>(smem_raw);                                    // [BP2_STAGES][TILE_FLOATS]
+    float2 *accs = reinterpret_cast<float2 *>(tiles + BP2_STAGES * TILE_FLOATS);           // [BZ / 2][256]
+    __shared__ SfView sview[BP2_STAGES];
+    __shared__ TileInfo tinfo[BP2_STAGES];
+    __shared__ __align__(8) uint64_t full[BP2_STAGES], empty[BP2_STAGES];
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tx = tid % BX, ty = tid / BX;
+    const int bzi = blockIdx.z % nbz, batch = blockIdx.z / nbz;
+    const int p0 = blockIdx.x * BX, q0 = blockIdx.y * BY, z0 = bzi * BZ;
+    const int p1 = min(p0 + BX, pr.nx) - 1, q1 = min(q0 + BY, pr.ny) - 1, z1 = min(z0 + BZ, pr.nz) - 1;
+    const int ip = p0 + tx, iq = q0 + ty;
+    const bool col_in = ip < pr.nx && iq < pr.ny;
+    const float p = (float)ip, q = (float)iq;
+    const int view_off = batch * view_count;
+    const int nzb = z1 - z0 + 1;                                 // voxels in this brick's z-run
+
+    for (int i = tid; i < (BZ / 2) * BRICK_THREADS; i += BRICK_THREADS) accs[i] = make_float2(0.0f, 0.0f);
+    for (int i = tid; i < BP2_STAGES * LM * TW; i += BRICK_THREADS)
+        tiles[(i / (LM * TW)) * TILE_FLOATS + TH * TW + i % (LM * TW)] = 0.0f;
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < BP2_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], BRICK_THREADS / 32); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // warp 0: stage view j into ring slot s (parameters, shadow, TMA) and arm full[s]
+    auto produce = [&](int j, int s) {
+        const SfView *gv = views + view_begin + (size_t)j * view_stride;
+        constexpr int W = (int)(sizeof(SfView) / 4);
+        for (int w = lane; w < W; w += 32)
+            reinterpret_cast<uint32_t *>(&sview[s])[w] = reinterpret_cast<const uint32_t *>(gv)[w];
+        __syncwarp();
+        TileInfo t = brick_shadow<ARC>(sview[s], pr, (float)p0, (float)p1, (float)q0, (float)q1, (float)z0, (float)z1, lane);
+        if (lane == 0) {
+            tinfo[s] = t;
+            if (t.live) {
+                mbar_expect_tx(&full[s], TW * TH * 4);              // arrive (release: the stores above) + tx count
+                tma_load_3d(tiles + s * TILE_FLOATS, &tmap, &full[s], t.k0, t.l0, view_off + j);
+            } else {
+                mbar_arrive(&full[s]);
+            }
+        }
+        __syncwarp();
+    };
+    auto coop_load = [&](float *dst, int k0, int l0, int j) {
+        const float *src = proj + (size_t)(view_off + j) * pr.nu * pr.nv;
+        for (int i = tid; i < TW * TH; i += BRICK_THREADS) {
+            const int r = i / TW, cidx = i - r * TW;
+            const int k = k0 + cidx, l = l0 + r;
+            const bool ok = k >= 0 && k < pr.nu && l >= 0 && l < pr.nv;
+            const float *gp = ok ? src + (size_t)l * pr.nu + k : src;
+            const int sz = ok ? 4 : 0;
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(smem_u32(dst + i)), "l"(gp), "r"(sz) : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+    };
+
+    if (warp == 0)
+        for (int d = 0; d < BP2_STAGES - 1 && j_lo + d < j_hi; ++d) produce(j_lo + d, d);
+
+    int s = 0, sp = BP2_STAGES - 1;           // slot of view j / of view j + BP2_STAGES - 1
+    uint32_t par = 0u;                        // phase parity of slot s's current use
+    for (int j = j_lo; j < j_hi; ++j) {
+        if (warp == 0 && j + BP2_STAGES - 1 < j_hi) {
+            // slot sp held view j - 1: every warp must have left it (its first use needs no wait)
+            if (j > j_lo) mbar_wait(&empty[sp], (uint32_t)(((j - 1 - j_lo) / BP2_STAGES) & 1));
+            produce(j + BP2_STAGES - 1, sp);
+        }
+        mbar_wait(&full[s], par);
+        const TileInfo t = tinfo[s];
+        if (t.live) {
+            const SfView v = sview[s];
+            float *tile = tiles + s * TILE_FLOATS;
+            uint32_t tile_a = smem_u32(tile);
+            asm volatile("" : "+r"(tile_a));
+            const float a_col = fmaf(q, v.aq, fmaf(p, v.ap, v.a0));
+            const float b_col = fmaf(q, v.bq, fmaf(p, v.bp, v.b0));
+            const float c_col = fmaf(q, v.cq, fmaf(p, v.cp, v.c0));
+            const float m_amp = fmaxf(fabsf(p + v.ep0), fabsf(q + v.eq0));
+            for (int bl = 0; bl < t.nbl; ++bl)
+                for (int bk = 0; bk < t.nbk; ++bk) {
+                    const int tk0 = t.k0 + bk * TW, tl0 = t.l0 + bl * TH;
+                    if (bk != 0 || bl != 0) {            // a shadow larger than one box (rare): block-wide staging
+                        __syncthreads();
+                        coop_load(tile, tk0, tl0, j);
+                        __syncthreads();
+                    }
+                    if (!col_in) continue;
+                    const int kmin = max(0, tk0), kmax = min(pr.nu - 1, tk0 + TW - 1);
+                    const int lmin = max(0, tl0), lmax = min(pr.nv - 1, tl0 + TH - 1);
+                    for (int zi = 0; zi < nzb; zi += 2) {
+                        const float2 z = p2((float)(z0 + zi), (float)(z0 + zi + 1));
+                        const float2 a = p2fma(z, p2s(v.az), p2s(a_col)), b = p2fma(z, p2s(v.bz), p2s(b_col));
+                        const float2 c = p2fma(z, p2s(v.cz), p2s(c_col));
+                        const float2 inv_a = p2rcp_nr(a);
+                        SfTrans2 T;
+                        sf_transaxial2<ARC, MODEL, BP2_SERIES>(v, a, b, inv_a, T, p, q);
+                        const float2 kf0 = p2add(T.kc, T.t0), kf3 = p2add(T.kc, T.t3);
+                        int kloA = max(kmin, (int)floorf(kf0.x)), khiA = min(kmax, (int)floorf(kf3.x));
+                        int kloB = max(kmin, (int)floorf(kf0.y)), khiB = min(kmax, (int)floorf(kf3.y));
+                        SfAxial2 A;
+                        sf_axial2<ARC, BP2_SERIES>(v, a, b, c, inv_a, A);
+                        const float2 lf0 = p2add(A.lc, A.tlo), lf1 = p2add(A.lc, A.thi);
+                        int lloA = max(lmin, (int)floorf(lf0.x)), lhiA = min(lmax, (int)floorf(lf1.x));
+                        int lloB = max(lmin, (int)floorf(lf0.y)), lhiB = min(lmax, (int)floorf(lf1.y));
+                        const bool liveA = kloA <= khiA && lloA <= lhiA;
+                        const bool liveB = kloB <= khiB && lloB <= lhiB && zi + 1 < nzb;
+                        if (!liveA && !liveB) continue;
+                        // a dead partner rides along with zero weights on a valid address
+                        if (!liveA) { kloA = kmin; khiA = kmin - 1; lloA = lmin; lhiA = lmin - 1; }
+                        if (!liveB) { kloB = kmin; khiB = kmin - 1; lloB = lmin; lhiB = lmin - 1; }
+                        float2 amp;
+                        if (RECON) {
+                            amp = p2(sf_recon_weight_s<ARC>(v, T.h01.x + T.w12.x + T.h23.x, A.thi.x - A.tlo.x, a.x, b.x),
+                                     sf_recon_weight_s<ARC>(v, T.h01.y + T.w12.y + T.h23.y, A.thi.y - A.tlo.y, a.y, b.y));
+                        } else {
+                            amp = sf_amplitude2(a, b, c, m_amp);
+                        }
+                        const int Kmax = max(khiA - kloA, khiB - kloB) + 1;
+                        const int Lmax = max(lhiA - lloA, lhiB - lloB) + 1;
+                        // the row loop runs over max(L_a, L_b) rows too: each footprint is cut at the lower edge of its
+                        // own last row, so the rows past it weigh exactly 0 (also where a box or the detector ends)
+                        A.thi = p2min(A.thi, p2sub(p2((float)(lhiA + 1), (float)(lhiB + 1)), A.lc));
+                        const float2 xi0 = p2sub(p2((float)kloA, (float)kloB), T.kc);
+                        const float2 xe = p2sub(p2((float)(khiA + 1), (float)(khiB + 1)), T.kc);   // last edge of each voxel
+                        const float2 g00 = sf_G2<MODEL>(T, xi0);
+                        float2 sum = p2s(0.0f);
+                        const uint32_t baseA = tile_a + 4u * (unsigned)((lloA - tl0) * TW + (kloA - tk0));
+                        const uint32_t baseB = tile_a + 4u * (unsigned)((lloB - tl0) * TW + (kloB - tk0));
+                        for (int lb = 0; lb < Lmax; lb += LM) {
+                            float2 f2[LM];
+                            sf_F2_run2<LM>(A, p2((float)(lloA + lb), (float)(lloB + lb)), f2);
+                            uint32_t ra = baseA + 4u * (unsigned)(lb * TW), rb = baseB + 4u * (unsigned)(lb * TW);
+                            float2 xi = xi0, g0 = g00;
+#pragma unroll 1
+                            for (int k = 0; k < Kmax; ++k, ra += 4, rb += 4) {
+                                const float ya0 = lds_f32(ra), ya1 = lds_f32(ra + 4 * TW), ya2 = lds_f32(ra + 8 * TW), ya3 = lds_f32(ra + 12 * TW);
+                                const float yb0 = lds_f32(rb), yb1 = lds_f32(rb + 4 * TW), yb2 = lds_f32(rb + 8 * TW), yb3 = lds_f32(rb + 12 * TW);
+                                xi = p2add(xi, p2s(1.0f));
+                                const float2 g1 = sf_G2<MODEL>(T, p2min(xi, xe));
+                                float2 sr = p2mul(f2[0], p2(ya0, yb0));
+                                sr = p2fma(f2[1], p2(ya1, yb1), sr);
+                                sr = p2fma(f2[2], p2(ya2, yb2), sr);
+                                sr = p2fma(f2[3], p2(ya3, yb3), sr);
+                                sum = p2fma(p2sub(g1, g0), sr, sum);
+                                g0 = g1;
+                            }
+                        }
+                        float2 *ap = accs + (zi >> 1) * BRICK_THREADS + tid;
+                        *ap = p2fma(amp, sum, *ap);
+                    }
+                }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[s]);
+        sp = s;
+        if (++s == BP2_STAGES) { s = 0; par ^= 1u; }
+    }
+    if (col_in) {
+        float *o = vol + (size_t)batch * pr.nx * pr.ny * pr.nz + ((size_t)z0 * pr.ny + iq) * pr.nx + ip;
+        for (int zi = 0; zi < nzb; ++zi) {
+            float *oz = o + (size_t)zi * pr.ny * pr.nx;
+            const float2 r2 = accs[(zi >> 1) * BRICK_THREADS + tid];
+            const float r = (zi & 1) ? r2.y : r2.x;
+            *oz = accumulate ? *oz + r : r;
+        }
+    }
+}
+
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -468,16 +680,23 @@ int launch_brick(const ct_geom *g, const float *d_proj, float *d_vol, int batch,
             use_tma = (dbg && dbg[0] >= '1' && dbg[0] <= '3') ? dbg[0] - '0' : 3;
     }
     const size_t smem = (size_t)(2 * TILE_FLOATS + BZ * BRICK_THREADS) * sizeof(float);
+    const size_t smem2 = (size_t)(BP2_STAGES * TILE_FLOATS + BZ * BRICK_THREADS) * sizeof(float);
     // untilted frames with small footprints (host bound): F1 weights live in registers along the z-run
     // (testing aids: CTSF_BP_NOHOIST / CTSF_BP_FORCEHOIST, as for the forward kernel)
     const bool hoist = !getenv("CTSF_BP_NOHOIST") &&
                        (g->fp_hoist_ok || (g->all_untilted && getenv("CTSF_BP_FORCEHOIST")));
+    // general frames: the packed two-voxel kernel (needs the TMA path); CTSF_BP_SCALAR=1 (testing aid) keeps the
+    // one-voxel-per-thread kernel
+    const bool packed = !hoist && use_tma == 3 && !getenv("CTSF_BP_SCALAR");
     auto kern = g->model == 1
         ? (hoist ? (recon ? bp_brick_kernel<ARC, 1, 1, 1> : bp_brick_kernel<ARC, 0, 1, 1>)
                  : (recon ? bp_brick_kernel<ARC, 1, 0, 1> : bp_brick_kernel<ARC, 0, 0, 1>))
         : (hoist ? (recon ? bp_brick_kernel<ARC, 1, 1, 0> : bp_brick_kernel<ARC, 0, 1, 0>)
                  : (recon ? bp_brick_kernel<ARC, 1, 0, 0> : bp_brick_kernel<ARC, 0, 0, 0>));
+    auto kern2 = g->model == 1 ? (recon ? bp_brick2_kernel<ARC, 1, 1> : bp_brick2_kernel<ARC, 0, 1>)
+                               : (recon ? bp_brick2_kernel<ARC, 1, 0> : bp_brick2_kernel<ARC, 0, 0>);
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (packed) cudaFuncSetAttribute(kern2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
     const int nbz = (pr.nz + BZ - 1) / BZ;
     int launches = 0;
     // The view loop is cut into chunks of ~96 MB of projections, one launch each (every launch after the
@@ -495,9 +714,13 @@ int launch_brick(const ct_geom *g, const float *d_proj, float *d_vol, int batch,
             if ((long)nb * nbz > 65535) nb = 65535 / nbz > 0 ? 65535 / nbz : 1;
             dim3 grid((pr.nx + BX - 1) / BX, (pr.ny + BY - 1) / BY, nbz * nb);
             // the tensor map addresses view (batch*vc + j): pass the buffer of image b0 by offsetting batch in-kernel
-            kern<<<grid, BRICK_THREADS, smem, st>>>(pr, g->d_bp, d_proj + (size_t)b0 * vc * pr.nv * pr.nu, tmap, b0 == 0 ? use_tma : 0,
-                                                    d_vol + (size_t)b0 * pr.nx * pr.ny * pr.nz, vb, vs, vc, j_lo, j_hi, nbz,
-                                                    accumulate || j_lo > 0);
+            if (packed && b0 == 0)
+                kern2<<<grid, BRICK_THREADS, smem2, st>>>(pr, g->d_bp, d_proj, tmap, d_vol, vb, vs, vc, j_lo, j_hi, nbz,
+                                                          accumulate || j_lo > 0);
+            else
+                kern<<<grid, BRICK_THREADS, smem, st>>>(pr, g->d_bp, d_proj + (size_t)b0 * vc * pr.nv * pr.nu, tmap, b0 == 0 ? use_tma : 0,
+                                                        d_vol + (size_t)b0 * pr.nx * pr.ny * pr.nz, vb, vs, vc, j_lo, j_hi, nbz,
+                                                        accumulate || j_lo > 0);
             ++launches;
             b0 += nb;
         }
