@@ -10,6 +10,14 @@ inputs resident in HBM; e2e = the same through ct_fp_sf_host / ct_bp_sf_host wit
 
 N > 1 (torchrun): every rank runs an independent replica of the workload (the path shards by
 batch/volume with no data-path collective), weak scaling, max-over-ranks time.
+`--shard views` instead splits the views of ONE workload over the ranks: A on each rank's
+shard of views with the volume replicated, A^T on the shard followed by one NCCL sum all-reduce of the volume;
+strong scaling.
+
+roofline.peak is MEASURED in the same run (ct_measure_fp32_peak: FMA-only kernel, before the timed region);
+roofline.achieved = algorithmic flops (FLOP_PER_UPDATE, a count of the method's arithmetic) /
+the dominant kernel's CUDA-event time; the flops the kernels actually execute (ncu op counts) and their DRAM
+traffic are read from profiles/measured_counts.json, which names the capture each number comes from.
 """
 import argparse
 import json
@@ -47,8 +55,18 @@ def peaks():
         p.update(hbm_gbs=float(m["hbm_gbs"]), sm_max_mhz=float(m.get("sm_max_mhz", 1965.0)), src="measured")
     except Exception:
         pass
-    p["fp32_tflops"] = N_SM * FP32_LANES_PER_SM * 2 * p["sm_max_mhz"] * 1e6 / 1e12
+    p["fp32_tflops_nominal"] = N_SM * FP32_LANES_PER_SM * 2 * p["sm_max_mhz"] * 1e6 / 1e12
     return p
+
+
+def measured_counts(config_index, algo):
+    """ncu-measured per-call counts of the hot kernels (executed fp32 flops, DRAM bytes), from the committed
+    profiles/measured_counts.json; every entry names the capture file it was read from.  None when absent."""
+    try:
+        m = json.load(open(os.path.join(ROOT, "profiles", "measured_counts.json")))
+        return m.get("%s_config%d" % (algo, config_index))
+    except Exception:
+        return None
 
 
 class ClockSampler:
@@ -157,6 +175,9 @@ def main():
                     help="voxel model: SF (separable footprint, the headline) or DD (distance-driven, row f4)")
     ap.add_argument("--fbp", action="store_true",
                     help="also time recon mode (row f2): ct_fbp_filter + ct_bp_sf_recon on the step's projections")
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "views"],
+                    help="N > 1: independent replicas (weak scaling, default) or ONE workload with its views sharded "
+                         "over the ranks, A^T followed by one NCCL all-reduce of the volume (strong scaling)")
     ap.add_argument("--view-stride", type=int, default=1,
                     help="profiling aid: use every S-th view only (ordered subset); not a bench value")
     args = ap.parse_args()
@@ -188,15 +209,28 @@ def main():
     sel = None if vs == 1 else (0, vs, n_sel)
     if vs > 1:
         args.no_e2e = True
+    shard_views = args.shard == "views"
+    if shard_views:
+        from paper_2503_16741_b200.geometry import shard_views as shard_of
+        sel = shard_of(c["n_views"], world, rank)       # this rank's contiguous block of views
+        n_sel = sel[2]
+        args.no_e2e = True
     y = torch.empty((batch, n_sel, c["nv"], c["nu"]), device="cuda", dtype=torch.float32)
     xb = torch.empty_like(x)
     stream = torch.cuda.current_stream()
     updates = float(W.n_updates(c)) * n_sel / c["n_views"]
+    # measured fp32 peak (FMA-only kernel), before the timed region, with the clock it ran at
+    peak_sampler = ClockSampler(local) if rank == 0 else None
+    peak_flops = [B.ct_measure_fp32_peak(k, stream.cuda_stream)[0] for k in (0, 1, 0, 1)]
+    peak_clocks = peak_sampler.stop() if peak_sampler else None
+    peak_scalar, peak_packed = max(peak_flops[0::2]) / 1e12, max(peak_flops[1::2]) / 1e12
 
     def step():
         geom.fp(x, views=sel, out=y)
         n1 = geom.last_launch_count()
         geom.bp(y, views=sel, out=xb)
+        if shard_views and world > 1:
+            dist.all_reduce(xb)                      # the path's one exchange step
         return n1 + geom.last_launch_count()
 
     def barrier():
@@ -219,6 +253,8 @@ def main():
         geom.bp(y, views=sel, out=xb)
         launches += geom.last_launch_count()
         ev[3 * i + 2].record(stream)
+        if shard_views and world > 1:
+            dist.all_reduce(xb)                      # NCCL, on the current stream
         ev[3 * i + 3].record(stream)
     barrier()
     clocks = sampler.stop() if sampler else None
@@ -230,7 +266,19 @@ def main():
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     total_ms = t.item()
     ms_per_step = total_ms / args.steps
-    value = world * 2.0 * updates / (ms_per_step * 1e-3) / 1e9
+    ar_ms = float(np.mean([ev[3 * i + 2].elapsed_time(ev[3 * i + 3]) for i in range(args.steps)]))
+    if shard_views:
+        # one workload over all ranks: whole-job updates / max-over-ranks time
+        value = 2.0 * float(W.n_updates(c)) / (ms_per_step * 1e-3) / 1e9
+        per_rank = torch.tensor([fp_ms, bp_ms, ar_ms], device="cuda", dtype=torch.float64)
+        gathered = [torch.zeros_like(per_rank) for _ in range(world)]
+        if world > 1:
+            dist.all_gather(gathered, per_rank)
+        else:
+            gathered = [per_rank]
+        per_rank_ms = [[round(v, 3) for v in t.tolist()] for t in gathered]
+    else:
+        value = world * 2.0 * updates / (ms_per_step * 1e-3) / 1e9
 
     # ---- recon mode (row f2), reported beside the headline, never part of it -------------------------------
     recon = None
@@ -288,35 +336,50 @@ def main():
         flop = FLOP_PER_UPDATE[args.config] * updates
         alg_bytes = 4.0 * (x.numel() + y.numel())
         dom, dom_ms = ("ct_fp_sf", fp_ms) if fp_ms >= bp_ms else ("ct_bp_sf", bp_ms)
-        traffic = None
-        try:
-            traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.txt"))).get(
-                "config%d" % args.config, {}).get(dom)
-        except Exception:
-            pass
+        mc = measured_counts(args.config, args.algo) or {}
+        mdom = mc.get(dom, {})
+        traffic = mdom.get("dram_bytes") if vs == 1 and not shard_views else None
         achieved = flop / (dom_ms * 1e-3) / 1e12
+        peak = max(peak_scalar, peak_packed)
         line = {
             "metric": metric_name(args.config), "value": value, "unit": "GUPS", "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "strong" if shard_views else "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": c["name"], "algo": args.algo, "index": args.config, "volume": [c["nz"], c["ny"], c["nx"]],
                        "views": n_sel, "detector": [c["nv"], c["nu"]], "batch": batch,
-                       "step": "1 x ct_fp_sf + 1 x ct_bp_sf", "updates_per_operator": updates,
-                       "l2": "inputs (%.0f MB) exceed the 126 MB L2; no flush" % (alg_bytes / 1e6),
-                       "parallelism": "replicas" if world > 1 else "single"},
+                       "step": "1 x ct_fp_sf + 1 x ct_bp_sf" + (" + all-reduce(volume)" if shard_views else ""),
+                       "updates_per_operator": updates,
+                       "l2": "inputs (%.0f MB) exceed the 126 MB L2; no flush" % (alg_bytes / 1e6)
+                             if alg_bytes > 126e6 else
+                             "inputs (%.1f MB) fit the 126 MB L2 and stay there between steps; no flush (small "
+                             "parity-test config, not the headline)" % (alg_bytes / 1e6),
+                       "parallelism": ("views sharded over %d ranks + 1 all-reduce" % world) if shard_views
+                                      else ("replicas" if world > 1 else "single")},
             "fp_ms": fp_ms, "bp_ms": bp_ms,
             "fp_gups": updates / (fp_ms * 1e-3) / 1e9, "bp_gups": updates / (bp_ms * 1e-3) / 1e9,
             "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "recon": recon,
-            "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": pk["fp32_tflops"],
-                         "unit": "TFLOP/s", "frac": achieved / pk["fp32_tflops"], "traffic": traffic,
-                         "peak_src": "148 SM x 128 fp32 lanes x 2 x %.0f MHz (MEASURED_PEAKS sm_max_mhz, %s)"
-                                     % (pk["sm_max_mhz"], pk["src"]),
+            "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak,
+                         "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
+                         "peak_src": "measured in this run by ct_measure_fp32_peak (FMA-only kernel, best of 2 x 3): "
+                                     "scalar FFMA %.2f, packed FFMA2 %.2f TFLOP/s at %s MHz; nominal 148 SM x 128 lanes x "
+                                     "2 x %.0f MHz = %.2f" % (peak_scalar, peak_packed,
+                                                              peak_clocks.get("sm_mhz") if peak_clocks else "?",
+                                                              pk["sm_max_mhz"], pk["fp32_tflops_nominal"]),
+                         "peak_scalar_ffma": peak_scalar, "peak_packed_ffma2": peak_packed,
                          "flop_per_update": FLOP_PER_UPDATE[args.config],
+                         "flop_per_update_src": "algorithmic count of S1-S5 per nominal update (DESIGN.md section 7)",
+                         "executed_flop_per_update": mdom.get("flop_per_update"),
+                         "executed_frac": (mdom["flop_per_update"] * updates / (dom_ms * 1e-3) / 1e12 / peak)
+                                          if mdom.get("flop_per_update") else None,
+                         "measured_counts_src": mdom.get("src"),
                          "hbm": {"algorithmic_bytes": alg_bytes, "achieved_gbs": alg_bytes / (dom_ms * 1e-3) / 1e9,
                                  "peak_gbs": pk["hbm_gbs"], "frac": alg_bytes / (dom_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
                                  "note": "algorithmic bytes / kernel time; the path is ALU-bound by >200x "
                                          "(DESIGN.md), so this fraction is small by construction"}},
         }
+        if shard_views:
+            line["shard"] = {"mode": "views", "per_rank_ms_fp_bp_allreduce": per_rank_ms}
         if world == 1 and not args.no_cpu:
             line["cpu_baseline"] = cpu_baseline(c, x_host)
             lf = line["cpu_baseline"]["live_fraction"]

@@ -69,10 +69,12 @@ typedef struct {
     int32_t algo;                /* voxel model of every operator of this geometry:
                                     CT_ALGO_SF = 0 separable footprint, trapezoid x rectangle ("volume-based");
                                     CT_ALGO_DD = 1 distance-driven ("face-based": the voxel's central face
-                                    perpendicular to the ray's dominant axis, rectangle x rectangle; R26) */
+                                    perpendicular to the ray's dominant axis, rectangle x rectangle; R26);
+                                    CT_ALGO_SFTT = 2 separable footprint with a TRAPEZOID axial factor (SF-TT, for cone
+                                    angles beyond ~10 degrees; R27; identical to SF in 2-D) */
 } ct_geom_desc_t;
 
-enum { CT_ALGO_SF = 0, CT_ALGO_DD = 1 };
+enum { CT_ALGO_SF = 0, CT_ALGO_DD = 1, CT_ALGO_SFTT = 2 };
 
 /* Validates `desc`, derives the per-view kernel parameters in float64, rounds them to fp32 and
  * uploads them to the current CUDA device.  The host arrays are copied; the caller may free them
@@ -85,7 +87,10 @@ CTSF_API ct_status_t ct_geom_destroy(ct_geom_t *geom);
 
 /* y = A x (Eq. 1).  d_vol: DEVICE, read, [batch][nz][ny][nx].
  * d_proj: DEVICE, written (every element exactly once), [batch][n_views][nv][nu].
- * Both 16-byte aligned, caller-owned, must not overlap.  Asynchronous on `stream`. */
+ * Both caller-owned, fp32-aligned, must not overlap (a 16-byte aligned projection buffer with nu % 4 == 0 lets the
+ * backprojector stage its tiles by TMA; other buffers take the cp.async path -- same results).  Asynchronous on
+ * `stream`; makes no allocator call once the geometry is warm (the scratch for the xy-transposed volume that views
+ * along x read is owned by the geometry, grown on first use and kept until ct_geom_destroy). */
 CTSF_API ct_status_t ct_fp_sf(const ct_geom_t *geom, const float *d_vol, float *d_proj,
                      int32_t batch, ct_stream_t stream);
 
@@ -123,9 +128,18 @@ CTSF_API ct_status_t ct_bp_sf_recon(const ct_geom_t *geom, const float *d_proj, 
 CTSF_API ct_status_t ct_bp_sf_recon_views(const ct_geom_t *geom, const float *d_proj, float *d_vol, int32_t batch,
                                  int32_t view_begin, int32_t view_stride, int32_t view_count, ct_stream_t stream);
 
+/* The whole filtered backprojection of a full 360-degree scan with equi-angular views (
+ * DESIGN.md reading R25): x = (pi / n_views) * ct_bp_sf_recon(ct_fbp_filter(p)), the angular weight folded into the
+ * filter.  d_proj: DEVICE, read, [batch][n_views][nv][nu]; d_work: DEVICE scratch of the same size (holds the
+ * filtered projections afterwards), must not alias d_proj; d_vol: DEVICE, written.  Asynchronous on `stream`. */
+CTSF_API ct_status_t ct_fbp_sf(const ct_geom_t *geom, const float *d_proj, float *d_work, float *d_vol,
+                      int32_t batch, ct_stream_t stream);
+
 /* End-to-end convenience with HOST buffers (pageable or pinned): allocates device buffers from the
  * stream-ordered pool, copies the input host->device, runs the operator, copies the result
- * device->host and synchronises `stream` before returning.  Same layouts as above. */
+ * device->host and synchronises `stream` before returning.  Same layouts as above; any fp32-aligned host pointers.
+ * 3-D, batch 1: copies and kernels of neighbouring view chunks overlap on a second stream owned by the geometry;
+ * calls on one geometry are serialised. */
 CTSF_API ct_status_t ct_fp_sf_host(const ct_geom_t *geom, const float *h_vol, float *h_proj,
                           int32_t batch, ct_stream_t stream);
 CTSF_API ct_status_t ct_bp_sf_host(const ct_geom_t *geom, const float *h_proj, float *h_vol,

@@ -41,7 +41,9 @@ typedef struct {
     const double *det_center;/* [n_views][3] */
     const double *det_u;     /* [n_views][3] */
     const double *det_v;     /* [n_views][3]; dim 2: ignored, taken as (0,0,1) */
-    int model;               /* 0: separable footprint SF-TR; 1: distance-driven DD (row f4, reading R26) */
+    int model;               /* 0: separable footprint SF-TR; 1: distance-driven DD (row f4, reading R26);
+                                2: SF-TT, trapezoid axial footprint; 3: SF-TT with a row-dependent polar amplitude
+                                (row f3, reading R27; oracle only -- measured against ray/box chords, not built on the GPU) */
 } sfo_geom;
 
 /* O1: per-view frame. */
@@ -106,7 +108,7 @@ static void sort4(double *a)
  * Returns 1 when the footprint touches the detector, 0 otherwise. */
 static int footprint(const sfo_geom *g, const sfo_frame *f, int ix, int iy, int iz,
                      int *k_lo, int *k_hi, double *F1, int *l_lo, int *l_hi, double *F2,
-                     double *amp, double *tau_out)
+                     double *amp, double *tau_out, double *sumF2_out)
 {
     /* voxel centre (R9) */
     double Pc[3] = { g->ox + (ix - 0.5*(g->nx - 1))*g->dx,
@@ -151,12 +153,59 @@ static int footprint(const sfo_geom *g, const sfo_frame *f, int ix, int iy, int 
         F1[k - klo] = (sfo_trap_cdf(tau, uk + 0.5*g->du) - sfo_trap_cdf(tau, uk - 0.5*g->du)) / g->du;
     }
     /* O5: axial footprint (R5) */
-    if (g->dim == 3) {
+    if (g->dim == 3 && g->model >= 2) {
+        /* R27 ("higher-cone-angle SF variants"): the axial footprint of a ray family at row
+         * coordinate t is the fraction of the in-plane chord (length l_theta, from the voxel's near point to its far
+         * point along the voxel-centre ray's in-plane direction) that lies between z_c - dz/2 and z_c + dz/2: a
+         * TRAPEZOID whose vertices are the row coordinates of (near, far) x (z_c -+ dz/2).  model 3 additionally
+         * evaluates the polar stretch |d| / |d_xy| of the amplitude per detector row instead of at the voxel centre. */
+        double exy[2] = { Pc[0]-f->S[0], Pc[1]-f->S[1] };
+        double nxy = sqrt(exy[0]*exy[0] + exy[1]*exy[1]);
+        double ux = exy[0]/nxy, uy = exy[1]/nxy;
+        double rx_ = g->dx / fabs(ux), ry_ = g->dy / fabs(uy);
+        double lth = rx_ < ry_ ? rx_ : ry_;
+        double xi[4]; int c4 = 0;
+        for (int sn = -1; sn <= 1; sn += 2)
+            for (int sz = -1; sz <= 1; sz += 2) {
+                double P[3] = { Pc[0] + sn*0.5*lth*ux, Pc[1] + sn*0.5*lth*uy, Pc[2] + sz*0.5*g->dz };
+                double s_unused;
+                if (!det_coords(g, f, P, &s_unused, &xi[c4])) return 0;
+                ++c4;
+            }
+        sort4(xi);
+        if (sumF2_out) *sumF2_out = 0.5*(xi[3] + xi[2] - xi[1] - xi[0]) / g->dv;   /* area of the trapezoid */
+        int llo = (int)floor(xi[0]/g->dv + 0.5*g->nv), lhi = (int)floor(xi[3]/g->dv + 0.5*g->nv);
+        if (llo < 0) llo = 0;
+        if (lhi > g->nv - 1) lhi = g->nv - 1;
+        *l_lo = llo; *l_hi = lhi;
+        if (llo > lhi) return 0;
+        double e3[3] = { Pc[0]-f->S[0], Pc[1]-f->S[1], Pc[2]-f->S[2] };
+        double polar_c = sqrt(e3[0]*e3[0] + e3[1]*e3[1] + e3[2]*e3[2]) / nxy;      /* |e| / |e_xy| at the voxel centre */
+        double sc, tc_unused;
+        det_coords(g, f, Pc, &sc, &tc_unused);
+        for (int l = llo; l <= lhi; ++l) {
+            double vl = (l - 0.5*(g->nv - 1))*g->dv;
+            F2[l - llo] = (sfo_trap_cdf(xi, vl + 0.5*g->dv) - sfo_trap_cdf(xi, vl - 0.5*g->dv)) / g->dv;
+            if (g->model == 3) {
+                /* ray from the source to the detector point (s of the voxel centre, row centre v_l) */
+                double d[3];
+                if (g->det_type == 0) {
+                    for (int q = 0; q < 3; ++q) d[q] = f->R*f->n[q] + (sc + f->Du)*f->u[q] + (vl + f->Dv)*f->v[q];
+                } else {
+                    double ga = sc / f->R;
+                    for (int q = 0; q < 3; ++q) d[q] = f->R*(sin(ga)*f->u[q] + cos(ga)*f->n[q]) + (vl + f->Dv)*f->v[q];
+                }
+                double polar_l = sqrt(d[0]*d[0] + d[1]*d[1] + d[2]*d[2]) / sqrt(d[0]*d[0] + d[1]*d[1]);
+                F2[l - llo] *= polar_l / polar_c;       /* the common amplitude below carries polar_c */
+            }
+        }
+    } else if (g->dim == 3) {
         double Pm[3] = { Pc[0], Pc[1], Pc[2] - 0.5*g->dz }, Pp[3] = { Pc[0], Pc[1], Pc[2] + 0.5*g->dz };
         double s_unused, ta, tb;
         if (!det_coords(g, f, Pm, &s_unused, &ta)) return 0;
         if (!det_coords(g, f, Pp, &s_unused, &tb)) return 0;
         double tlo = ta < tb ? ta : tb, thi = ta < tb ? tb : ta;
+        if (sumF2_out) *sumF2_out = (thi - tlo) / g->dv;
         int llo = (int)floor(tlo/g->dv + 0.5*g->nv), lhi = (int)floor(thi/g->dv + 0.5*g->nv);
         if (llo < 0) llo = 0;
         if (lhi > g->nv - 1) lhi = g->nv - 1;
@@ -170,6 +219,7 @@ static int footprint(const sfo_geom *g, const sfo_frame *f, int ix, int iy, int 
         }
     } else {
         *l_lo = 0; *l_hi = 0; F2[0] = 1.0;                                  /* R18 */
+        if (sumF2_out) *sumF2_out = 1.0;
     }
     /* O6: amplitude along the voxel-centre ray (R2, R14) */
     double e[3] = { Pc[0]-f->S[0], Pc[1]-f->S[1], g->dim == 3 ? Pc[2]-f->S[2] : 0.0 };
@@ -188,7 +238,7 @@ int sfo_footprint(const sfo_geom *g, int view, int ix, int iy, int iz,
 {
     sfo_frame f; make_frame(g, view, &f);
     rng_out[0] = 0; rng_out[1] = -1; rng_out[2] = 0; rng_out[3] = -1;
-    return footprint(g, &f, ix, iy, iz, &rng_out[0], &rng_out[1], F1, &rng_out[2], &rng_out[3], F2, amp, tau_out);
+    return footprint(g, &f, ix, iy, iz, &rng_out[0], &rng_out[1], F1, &rng_out[2], &rng_out[3], F2, amp, tau_out, NULL);
 }
 
 /* Detector coordinates of a world point in one view (for the brute-force pins). */
@@ -207,7 +257,7 @@ static void fp_view_slab(const sfo_geom *g, const sfo_frame *f, const double *vo
             for (int ix = 0; ix < g->nx; ++ix) {
                 double xv = vol[((size_t)iz*g->ny + iy)*g->nx + ix];
                 int klo, khi, llo, lhi; double amp;
-                if (!footprint(g, f, ix, iy, iz, &klo, &khi, F1, &llo, &lhi, F2, &amp, NULL)) continue;
+                if (!footprint(g, f, ix, iy, iz, &klo, &khi, F1, &llo, &lhi, F2, &amp, NULL, NULL)) continue;
                 for (int l = llo; l <= lhi; ++l)
                     for (int k = klo; k <= khi; ++k)
                         y[(size_t)l*g->nu + k] += amp * F1[k - klo] * F2[l - llo] * xv;
@@ -269,7 +319,7 @@ static double bp_voxel(const sfo_geom *g, const sfo_frame *frames, const double 
     double acc = 0.0;
     for (int j = 0; j < n_sel; ++j) {
         int klo, khi, llo, lhi; double amp;
-        if (!footprint(g, &frames[j], ix, iy, iz, &klo, &khi, F1, &llo, &lhi, F2, &amp, NULL)) continue;
+        if (!footprint(g, &frames[j], ix, iy, iz, &klo, &khi, F1, &llo, &lhi, F2, &amp, NULL, NULL)) continue;
         const double *y = proj + ncell*j;
         for (int l = llo; l <= lhi; ++l)
             for (int k = klo; k <= khi; ++k)
@@ -356,15 +406,9 @@ static double bp_voxel_recon(const sfo_geom *g, const sfo_frame *frames, const d
     double acc = 0.0;
     for (int j = 0; j < n_sel; ++j) {
         const sfo_frame *f = &frames[j];
-        int klo, khi, llo, lhi; double amp, tau[4];
-        if (!footprint(g, f, ix, iy, iz, &klo, &khi, F1, &llo, &lhi, F2, &amp, tau)) continue;
-        double sumF1 = 0.5*(tau[3] + tau[2] - tau[1] - tau[0]) / g->du, sumF2 = 1.0;
-        if (g->dim == 3) {
-            double Pm[3] = { Pc[0], Pc[1], Pc[2] - 0.5*g->dz }, Pp[3] = { Pc[0], Pc[1], Pc[2] + 0.5*g->dz };
-            double s_unused, ta, tb;
-            det_coords(g, f, Pm, &s_unused, &ta); det_coords(g, f, Pp, &s_unused, &tb);
-            sumF2 = fabs(tb - ta) / g->dv;
-        }
+        int klo, khi, llo, lhi; double amp, tau[4], sumF2 = 1.0;
+        if (!footprint(g, f, ix, iy, iz, &klo, &khi, F1, &llo, &lhi, F2, &amp, tau, &sumF2)) continue;
+        double sumF1 = 0.5*(tau[3] + tau[2] - tau[1] - tau[0]) / g->du;     /* sumF2: the axial factor's own unclipped sum */
         double w[3] = { Pc[0]-f->S[0], Pc[1]-f->S[1], Pc[2]-f->S[2] };
         double a = dot3(w, f->n), b = dot3(w, f->u);
         double Sn = dot3(f->S, f->n), Su = dot3(f->S, f->u);
@@ -439,7 +483,7 @@ int sfo_bp_voxels_f32(const sfo_geom *g, const float *proj, const int *ijk, int 
             double acc = 0.0;
             for (int j = 0; j < g->n_views; ++j) {
                 int klo, khi, llo, lhi; double amp;
-                if (!footprint(g, &frames[j], ijk[3*i], ijk[3*i+1], ijk[3*i+2], &klo, &khi, F1, &llo, &lhi, F2, &amp, NULL)) continue;
+                if (!footprint(g, &frames[j], ijk[3*i], ijk[3*i+1], ijk[3*i+2], &klo, &khi, F1, &llo, &lhi, F2, &amp, NULL, NULL)) continue;
                 const float *y = proj + ncell*j;
                 for (int l = llo; l <= lhi; ++l)
                     for (int k = klo; k <= khi; ++k)
@@ -465,7 +509,7 @@ double sfo_live_fraction(const sfo_geom *g, int vox_stride, int view_stride)
             for (int iy = 0; iy < g->ny; iy += vox_stride)
                 for (int ix = 0; ix < g->nx; ix += vox_stride) {
                     int klo, khi, llo, lhi; double amp;
-                    live += footprint(g, &f, ix, iy, iz, &klo, &khi, F1, &llo, &lhi, F2, &amp, NULL);
+                    live += footprint(g, &f, ix, iy, iz, &klo, &khi, F1, &llo, &lhi, F2, &amp, NULL, NULL);
                     ++total;
                 }
     }

@@ -76,7 +76,8 @@ def _f64(a):
 class Oracle:
     """One scan geometry.  `g` is a plain dict with the keys of the problem description:
     dim, nx, ny, nz, dx, dy, dz, ox, oy, oz, nu, nv, du, dv, det_type ('flat'|'arc' or 0|1),
-    src, det_center, det_u, det_v (each [n_views, 3], float64); optional algo 'SF' (default) | 'DD'."""
+    src, det_center, det_u, det_v (each [n_views, 3], float64); optional algo 'SF' (default) | 'DD' | 'SF-TT' | 'SF-TT-A2'
+    (the last two: row f3 variants, oracle only)."""
 
     def __init__(self, g):
         self.lib = _load()
@@ -100,7 +101,7 @@ class Oracle:
                        int(det), self.n_views,
                        self.src.ctypes.data, self.dc.ctypes.data,
                        self.du_vec.ctypes.data, self.dv_vec.ctypes.data,
-                       {"SF": 0, "DD": 1}.get(g.get("algo", "SF"), g.get("algo", 0)))
+                       {"SF": 0, "DD": 1, "SF-TT": 2, "SF-TT-A2": 3}.get(g.get("algo", "SF"), g.get("algo", 0)))
         self.threads = 0
 
     # -- pins ------------------------------------------------------------------------------

@@ -17,7 +17,7 @@ STATUS_NAMES = {0: "CT_OK", 1: "CT_ERR_INVALID_ARG", 2: "CT_ERR_GEOMETRY", 3: "C
                 4: "CT_ERR_ALLOC", 5: "CT_ERR_CUDA"}
 EXPORTS = ("ct_geom_create", "ct_geom_destroy", "ct_fp_sf", "ct_bp_sf", "ct_fp_sf_views", "ct_bp_sf_views",
            "ct_fp_sf_host", "ct_bp_sf_host", "ct_fbp_filter", "ct_fbp_filter_views", "ct_bp_sf_recon",
-           "ct_bp_sf_recon_views", "ct_measure_fp32_peak", "ct_last_launch_count", "ct_status_string")
+           "ct_bp_sf_recon_views", "ct_fbp_sf", "ct_measure_fp32_peak", "ct_last_launch_count", "ct_status_string")
 
 
 class CtError(RuntimeError):
@@ -61,12 +61,15 @@ def lib():
         L.ct_bp_sf_recon.argtypes = [P, P, P, I, P]
         L.ct_fbp_filter_views.argtypes = [P, P, P, I, I, I, I, P]
         L.ct_bp_sf_recon_views.argtypes = [P, P, P, I, I, I, I, P]
+        L.ct_fbp_sf.argtypes = [P, P, P, P, I, P]
+        L.ctsf_debug_set.argtypes = [ctypes.c_char_p, ctypes.c_double]
+        L.ctsf_debug_set.restype = ctypes.c_int
         L.ct_measure_fp32_peak.argtypes = [I, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), P]
         L.ct_last_launch_count.argtypes = [P]
         L.ct_last_launch_count.restype = I
         L.ct_status_string.argtypes = [ctypes.c_int]
         L.ct_status_string.restype = ctypes.c_char_p
-        for name in EXPORTS[:13]:
+        for name in EXPORTS[:14]:
             getattr(L, name).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -83,7 +86,7 @@ def _check(status, what):
 
 def ct_geom_create(g):
     """g: dict with the ct_geom_desc_t keys (det_type 'flat'|'arc' or 0|1; vectors as [n_views,3]
-    float64 arrays; optional algo 'SF' (default) | 'DD').  Returns an opaque handle (int) for the calls below."""
+    float64 arrays; optional algo 'SF' (default) | 'DD' | 'SF-TT').  Returns an opaque handle (int) for the calls below."""
     src = np.ascontiguousarray(g["src"], dtype=np.float64).reshape(-1, 3)
     dc = np.ascontiguousarray(g["det_center"], dtype=np.float64).reshape(-1, 3)
     du = np.ascontiguousarray(g["det_u"], dtype=np.float64).reshape(-1, 3)
@@ -99,7 +102,7 @@ def ct_geom_create(g):
                        int(g["nu"]), int(g.get("nv", 1)), float(g["du"]), float(g.get("dv", 1.0)),
                        int(det), int(n_views), src.ctypes.data, dc.ctypes.data, du.ctypes.data,
                        None if dv is None else dv.ctypes.data,
-                       int({"SF": 0, "DD": 1}.get(g.get("algo", "SF"), g.get("algo", 0))))
+                       int({"SF": 0, "DD": 1, "SF-TT": 2}.get(g.get("algo", "SF"), g.get("algo", 0))))
     out = ctypes.c_void_p()
     _check(lib().ct_geom_create(ctypes.byref(d), ctypes.byref(out)), "ct_geom_create")
     return out.value
@@ -153,6 +156,17 @@ def ct_fbp_filter(handle, d_proj, d_out, batch, stream=0):
 
 def ct_bp_sf_recon(handle, d_proj, d_vol, batch, stream=0):
     _check(lib().ct_bp_sf_recon(handle, d_proj, d_vol, batch, stream), "ct_bp_sf_recon")
+
+
+def ct_fbp_sf(handle, d_proj, d_work, d_vol, batch, stream=0):
+    _check(lib().ct_fbp_sf(handle, d_proj, d_work, d_vol, int(batch), stream), "ct_fbp_sf")
+
+
+def debug_set(name, value=1):
+    """Testing aid (ctsf_debug_set, not part of include/ctsf.h): force a rarely taken code path of the launchers;
+    debug_set('reset') restores the defaults.  Used by tests only."""
+    if lib().ctsf_debug_set(name.encode(), float(value)) != 0:
+        raise KeyError(name)
 
 
 def ct_measure_fp32_peak(kind=0, stream=0):

@@ -5,6 +5,7 @@
 #include <cmath>
 #include <mutex>
 #include <new>
+#include <string>
 
 #include "ctsf_internal.h"
 
@@ -49,15 +50,15 @@ ct_status_t check_call(const ct_geom *g, const void *a, const void *b, int batch
     if (!a || !b) return CT_ERR_INVALID_ARG;
     if (vc < 0 || vs < 1 || vb < 0) return CT_ERR_INVALID_ARG;
     if (vc > 0 && (long)vb + (long)(vc - 1) * vs >= g->prob.n_views) return CT_ERR_INVALID_ARG;
-    if (((uintptr_t)a | (uintptr_t)b) & 15u) return CT_ERR_INVALID_ARG;
-    return CT_OK;
+    if (((uintptr_t)a | (uintptr_t)b) & 3u) return CT_ERR_INVALID_ARG;     // fp32 elements; 16-byte alignment of the
+    return CT_OK;                                                            // projections only enables the TMA path
 }
 
 ct_status_t zero_volume(const ct_geom *g, float *d_vol, int batch, ct_stream_t stream)
 {
     const size_t n = (size_t)batch * g->prob.nx * g->prob.ny * g->prob.nz;
     if (cudaMemsetAsync(d_vol, 0, n * sizeof(float), (cudaStream_t)stream) != cudaSuccess) { cudaGetLastError(); return CT_ERR_CUDA; }
-    const_cast<ct_geom *>(g)->last_launches.store(0);
+    g->last_launches.store(0);
     return CT_OK;
 }
 
@@ -78,7 +79,58 @@ void ctsf_free_async(void *p, void *stream)
     if (p) cudaFreeAsync(p, (cudaStream_t)stream);
 }
 
+CtsfDebug g_ctsf_debug;
+
+void *ctsf_scratch_acquire(const ct_geom *g, size_t bytes, void *stream)
+{
+    std::lock_guard<std::mutex> lock(g->scratch_mu);
+    for (auto &sc : g->scratch) {
+        if (sc.bytes < bytes || !sc.ptr) continue;
+        // free for this call: same stream (ordered behind the previous use), or the previous use has completed
+        if (sc.stream == stream || (sc.done && cudaEventQuery((cudaEvent_t)sc.done) == cudaSuccess)) {
+            sc.stream = stream;
+            return sc.ptr;
+        }
+    }
+    cudaGetLastError();                     // cudaEventQuery's cudaErrorNotReady is not an error here
+    ct_geom::Scratch sc;
+    if (cudaMalloc(&sc.ptr, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    cudaEvent_t ev = nullptr;
+    if (cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); cudaFree(sc.ptr); return nullptr; }
+    sc.bytes = bytes; sc.stream = stream; sc.done = ev;
+    g->scratch.push_back(sc);
+    return sc.ptr;
+}
+
+void ctsf_scratch_release(const ct_geom *g, void *ptr, void *stream)
+{
+    std::lock_guard<std::mutex> lock(g->scratch_mu);
+    for (auto &sc : g->scratch)
+        if (sc.ptr == ptr) { cudaEventRecord((cudaEvent_t)sc.done, (cudaStream_t)stream); return; }
+}
+
 extern "C" {
+
+// Testing aid, deliberately NOT declared in include/ctsf.h: sets one switch of CtsfDebug by name (see ctsf_internal.h).
+// Returns 0, or -1 for an unknown name.  Not thread-safe against running calls.
+CTSF_API int ctsf_debug_set(const char *name, double value)
+{
+    if (!name) return -1;
+    const std::string n(name);
+    CtsfDebug &d = g_ctsf_debug;
+    if (n == "reset") d = CtsfDebug();
+    else if (n == "fp_pad") d.fp_pad = (float)value;
+    else if (n == "fp_nohoist") d.fp_nohoist = (int)value;
+    else if (n == "fp_forcehoist") d.fp_forcehoist = (int)value;
+    else if (n == "fp_serial") d.fp_serial = (int)value;
+    else if (n == "bp_nohoist") d.bp_nohoist = (int)value;
+    else if (n == "bp_forcehoist") d.bp_forcehoist = (int)value;
+    else if (n == "bp_tma") d.bp_tma = (int)value;
+    else if (n == "bp_chunk") d.bp_chunk = (int)value;
+    else if (n == "bp_scalar") d.bp_scalar = (int)value;
+    else return -1;
+    return 0;
+}
 
 ct_status_t ct_geom_create(const ct_geom_desc_t *d, ct_geom_t **out)
 {
@@ -91,7 +143,7 @@ ct_status_t ct_geom_create(const ct_geom_desc_t *d, ct_geom_t **out)
     if (d->dim == 3 && (!finite_pos(d->dz) || !finite_pos(d->dv))) return CT_ERR_INVALID_ARG;
     if (!std::isfinite(d->ox) || !std::isfinite(d->oy) || (d->dim == 3 && !std::isfinite(d->oz))) return CT_ERR_INVALID_ARG;
     if (d->det_type != 0 && d->det_type != 1) return CT_ERR_INVALID_ARG;
-    if (d->algo != CT_ALGO_SF && d->algo != CT_ALGO_DD) return CT_ERR_INVALID_ARG;
+    if (d->algo != CT_ALGO_SF && d->algo != CT_ALGO_DD && d->algo != CT_ALGO_SFTT) return CT_ERR_INVALID_ARG;
     if (!d->src || !d->det_center || !d->det_u || (d->dim == 3 && !d->det_v)) return CT_ERR_INVALID_ARG;
     if ((double)d->nx * d->ny * d->nz >= 2147483648.0 || (double)d->nu * d->nv * d->n_views >= 2147483648.0 * 4)
         return CT_ERR_UNSUPPORTED;
@@ -138,14 +190,19 @@ ct_status_t ct_geom_destroy(ct_geom_t *g)
     if (!g) return CT_OK;
     if (g->d_bp) cudaFree(g->d_bp);
     if (g->d_fp) cudaFree(g->d_fp);
-    delete g;
-    {
-        int dev = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < MAX_DEV) {
-            std::lock_guard<std::mutex> lock(g_pool_mu);
-            if (g_pool[dev]) cudaMemPoolTrimTo(g_pool[dev], 0);      // hand cached scratch back
-        }
+    for (auto &sc : g->scratch) {
+        if (sc.ptr) cudaFree(sc.ptr);                                 // synchronises with pending work on it
+        if (sc.done) cudaEventDestroy((cudaEvent_t)sc.done);
     }
+    if (g->host_copy_stream) cudaStreamDestroy((cudaStream_t)g->host_copy_stream);
+    for (void *e : g->host_events) if (e) cudaEventDestroy((cudaEvent_t)e);
+    const int dev = g->device;
+    delete g;
+    if (dev >= 0 && dev < MAX_DEV) {
+        std::lock_guard<std::mutex> lock(g_pool_mu);
+        if (g_pool[dev]) cudaMemPoolTrimTo(g_pool[dev], 0);          // hand the host-buffer operators' cached buffers back
+    }
+    cudaGetLastError();
     return CT_OK;
 }
 
@@ -154,10 +211,10 @@ ct_status_t ct_fp_sf_views(const ct_geom_t *g, const float *d_vol, float *d_proj
 {
     ct_status_t st = check_call(g, d_vol, d_proj, batch, vb, vs, vc, false, true);
     if (st != CT_OK) return st;
-    if (vc == 0) { const_cast<ct_geom *>(g)->last_launches.store(0); return CT_OK; }     // nothing to write
+    if (vc == 0) { g->last_launches.store(0); return CT_OK; }     // nothing to write
     int n = ctsf_launch_fp(g, d_vol, d_proj, batch, vb, vs, vc, stream);
     if (n < 0) return CT_ERR_CUDA;
-    const_cast<ct_geom *>(g)->last_launches.store(n);
+    g->last_launches.store(n);
     return CT_OK;
 }
 
@@ -169,7 +226,7 @@ ct_status_t ct_bp_sf_views(const ct_geom_t *g, const float *d_proj, float *d_vol
     if (vc == 0) return zero_volume(g, d_vol, batch, stream);                            // empty sum
     int n = ctsf_launch_bp(g, d_proj, d_vol, batch, vb, vs, vc, stream);
     if (n < 0) return CT_ERR_CUDA;
-    const_cast<ct_geom *>(g)->last_launches.store(n);
+    g->last_launches.store(n);
     return CT_OK;
 }
 
@@ -181,7 +238,7 @@ ct_status_t ct_bp_sf_recon_views(const ct_geom_t *g, const float *d_proj, float 
     if (vc == 0) return zero_volume(g, d_vol, batch, stream);
     int n = ctsf_launch_bp(g, d_proj, d_vol, batch, vb, vs, vc, stream, 0, 1);
     if (n < 0) return CT_ERR_CUDA;
-    const_cast<ct_geom *>(g)->last_launches.store(n);
+    g->last_launches.store(n);
     return CT_OK;
 }
 
@@ -196,11 +253,11 @@ ct_status_t ct_fbp_filter_views(const ct_geom_t *g, const float *d_proj, float *
 {
     ct_status_t st = check_call(g, d_proj, d_out, batch, vb, vs, vc, true, true);
     if (st != CT_OK) return st;
-    if (vc == 0) { const_cast<ct_geom *>(g)->last_launches.store(0); return CT_OK; }
+    if (vc == 0) { g->last_launches.store(0); return CT_OK; }
     if (d_proj == d_out) return CT_ERR_INVALID_ARG;           // not in place: every output reads the whole row
     int n = ctsf_launch_filter(g, d_proj, d_out, batch, vb, vs, vc, stream);
     if (n < 0) return CT_ERR_CUDA;
-    const_cast<ct_geom *>(g)->last_launches.store(n);
+    g->last_launches.store(n);
     return CT_OK;
 }
 
@@ -208,6 +265,23 @@ ct_status_t ct_fbp_filter(const ct_geom_t *g, const float *d_proj, float *d_out,
 {
     if (!g) return CT_ERR_INVALID_ARG;
     return ct_fbp_filter_views(g, d_proj, d_out, batch, 0, 1, g->prob.n_views, stream);
+}
+
+ct_status_t ct_fbp_sf(const ct_geom_t *g, const float *d_proj, float *d_work, float *d_vol, int32_t batch, ct_stream_t stream)
+{
+    if (!g) return CT_ERR_INVALID_ARG;
+    const int vc = g->prob.n_views;
+    ct_status_t st = check_call(g, d_proj, d_work, batch, 0, 1, vc, true, true);
+    if (st == CT_OK) st = check_call(g, d_work, d_vol, batch, 0, 1, vc, true, false);
+    if (st != CT_OK) return st;
+    if (d_proj == d_work) return CT_ERR_INVALID_ARG;
+    const double PI = 3.14159265358979323846;
+    const int n1 = ctsf_launch_filter(g, d_proj, d_work, batch, 0, 1, vc, stream, PI / (double)vc);     // reading R25
+    if (n1 < 0) return CT_ERR_CUDA;
+    const int n2 = ctsf_launch_bp(g, d_work, d_vol, batch, 0, 1, vc, stream, 0, 1);
+    if (n2 < 0) return CT_ERR_CUDA;
+    g->last_launches.store(n1 + n2);
+    return CT_OK;
 }
 
 ct_status_t ct_fp_sf(const ct_geom_t *g, const float *d_vol, float *d_proj, int32_t batch, ct_stream_t stream)
@@ -226,6 +300,8 @@ ct_status_t ct_bp_sf(const ct_geom_t *g, const float *d_proj, float *d_vol, int3
 // one chunk overlaps the kernel of its neighbour on a second stream (A: the projections of chunk c
 // go home while chunk c+1 is computed; A^T: chunk c+1 arrives while chunk c is backprojected into the
 // volume, every chunk after the first adding to it).  Other shapes: copy in, run, copy out.
+// The copy stream and the events belong to the geometry (made on first use, reused by every call); the volume
+// is transposed once per call, not once per chunk.  One host-buffer call per geometry at a time.
 static ct_status_t host_op(const ct_geom_t *g, const float *h_in, float *h_out, int32_t batch, ct_stream_t stream, bool fwd)
 {
     if (!g || !h_in || !h_out || batch < 1) return CT_ERR_INVALID_ARG;
@@ -233,71 +309,87 @@ static ct_status_t host_op(const ct_geom_t *g, const float *h_in, float *h_out, 
     const SfProblem &pr = g->prob;
     const size_t cells = (size_t)pr.nv * pr.nu;
     const size_t nvol = (size_t)batch * pr.nx * pr.ny * pr.nz, nproj = (size_t)batch * pr.n_views * cells;
-    float *d_vol = nullptr, *d_proj = nullptr;
-    d_vol = (float *)ctsf_alloc_async(nvol * sizeof(float), st);
+    std::lock_guard<std::mutex> host_lock(g->host_mu);
+    float *d_vol = (float *)ctsf_alloc_async(nvol * sizeof(float), st);
     if (!d_vol) return CT_ERR_ALLOC;
-    d_proj = (float *)ctsf_alloc_async(nproj * sizeof(float), st);
+    float *d_proj = (float *)ctsf_alloc_async(nproj * sizeof(float), st);
     if (!d_proj) { ctsf_free_async(d_vol, st); return CT_ERR_ALLOC; }
     ct_status_t rc = CT_OK;
     int launches = 0;
-    const int n_chunks = (pr.dim == 3 && batch == 1) ? (pr.n_views >= 64 ? 8 : (pr.n_views >= 8 ? 2 : 1)) : 1;
+    constexpr int MAX_CHUNKS = 8;
+    const int n_chunks = (pr.dim == 3 && batch == 1) ? (pr.n_views >= 64 ? MAX_CHUNKS : (pr.n_views >= 8 ? 2 : 1)) : 1;
+    auto ok = [&](cudaError_t e) { if (e != cudaSuccess && rc == CT_OK) rc = CT_ERR_CUDA; return e == cudaSuccess; };
     if (n_chunks == 1) {
         const float *d_in = fwd ? d_vol : d_proj;
         float *d_out = fwd ? d_proj : d_vol;
         const size_t n_in = fwd ? nvol : nproj, n_out = fwd ? nproj : nvol;
-        if (cudaMemcpyAsync((void *)d_in, h_in, n_in * sizeof(float), cudaMemcpyHostToDevice, st) != cudaSuccess) rc = CT_ERR_CUDA;
-        if (rc == CT_OK) rc = fwd ? ct_fp_sf(g, d_in, d_out, batch, stream) : ct_bp_sf(g, d_in, d_out, batch, stream);
-        launches = g->last_launches.load();
-        if (rc == CT_OK && cudaMemcpyAsync(h_out, d_out, n_out * sizeof(float), cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = CT_ERR_CUDA;
-    } else {
-        cudaStream_t cs = nullptr;                      // copy stream
-        cudaEvent_t ev[8] = {}, start = nullptr;
-        if (cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking) != cudaSuccess) rc = CT_ERR_CUDA;
-        if (rc == CT_OK && cudaEventCreateWithFlags(&start, cudaEventDisableTiming) != cudaSuccess) rc = CT_ERR_CUDA;
-        for (int c = 0; c < n_chunks && rc == CT_OK; ++c)
-            if (cudaEventCreateWithFlags(&ev[c], cudaEventDisableTiming) != cudaSuccess) rc = CT_ERR_CUDA;
+        ok(cudaMemcpyAsync((void *)d_in, h_in, n_in * sizeof(float), cudaMemcpyHostToDevice, st));
         if (rc == CT_OK) {
+            const int n = fwd ? ctsf_launch_fp(g, d_in, d_out, batch, 0, 1, pr.n_views, stream)
+                              : ctsf_launch_bp(g, d_in, d_out, batch, 0, 1, pr.n_views, stream);
+            if (n < 0) rc = CT_ERR_CUDA; else launches = n;
+        }
+        if (rc == CT_OK) ok(cudaMemcpyAsync(h_out, d_out, n_out * sizeof(float), cudaMemcpyDeviceToHost, st));
+    } else {
+        if (!g->host_copy_stream) {
+            cudaStream_t cs = nullptr;
+            if (ok(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking))) g->host_copy_stream = cs;
+            g->host_events.assign(MAX_CHUNKS + 1, nullptr);
+            for (auto &e : g->host_events) {
+                cudaEvent_t ev = nullptr;
+                if (ok(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming))) e = ev;
+            }
+        }
+        cudaStream_t cs = (cudaStream_t)g->host_copy_stream;
+        float *d_volT = nullptr;
+        if (rc == CT_OK) {
+            cudaEvent_t start = (cudaEvent_t)g->host_events[MAX_CHUNKS];
             // the copy stream may not touch the buffers before `st` has reached this call (allocation order)
-            cudaEventRecord(start, st);
-            cudaStreamWaitEvent(cs, start, 0);
-            if (fwd && cudaMemcpyAsync(d_vol, h_in, nvol * sizeof(float), cudaMemcpyHostToDevice, st) != cudaSuccess) rc = CT_ERR_CUDA;
+            ok(cudaEventRecord(start, st));
+            ok(cudaStreamWaitEvent(cs, start, 0));
+            if (fwd) {
+                ok(cudaMemcpyAsync(d_vol, h_in, nvol * sizeof(float), cudaMemcpyHostToDevice, st));
+                if (rc == CT_OK && ctsf_fp_needs_transpose(g, 0, 1, pr.n_views)) {
+                    d_volT = (float *)ctsf_scratch_acquire(g, nvol * sizeof(float), stream);
+                    const int n = d_volT ? ctsf_fp_transpose(g, d_vol, d_volT, 1, stream) : -1;
+                    if (n < 0) rc = d_volT ? CT_ERR_CUDA : CT_ERR_ALLOC; else launches += n;
+                }
+            }
         }
         for (int c = 0; c < n_chunks && rc == CT_OK; ++c) {
             const int v0 = (int)((long)pr.n_views * c / n_chunks), v1 = (int)((long)pr.n_views * (c + 1) / n_chunks);
             const size_t off = (size_t)v0 * cells, cnt = (size_t)(v1 - v0) * cells;
+            cudaEvent_t ev = (cudaEvent_t)g->host_events[c];
             if (fwd) {
-                rc = ct_fp_sf_views(g, d_vol, d_proj + off, 1, v0, 1, v1 - v0, stream);
-                launches += g->last_launches.load();
-                cudaEventRecord(ev[c], st);
-                cudaStreamWaitEvent(cs, ev[c], 0);
-                if (rc == CT_OK && cudaMemcpyAsync(h_out + off, d_proj + off, cnt * sizeof(float), cudaMemcpyDeviceToHost, cs) != cudaSuccess) rc = CT_ERR_CUDA;
+                const int n = ctsf_launch_fp(g, d_vol, d_proj + off, 1, v0, 1, v1 - v0, stream, d_volT);
+                if (n < 0) { rc = CT_ERR_CUDA; break; }
+                launches += n;
+                ok(cudaEventRecord(ev, st));
+                ok(cudaStreamWaitEvent(cs, ev, 0));
+                ok(cudaMemcpyAsync(h_out + off, d_proj + off, cnt * sizeof(float), cudaMemcpyDeviceToHost, cs));
             } else {
-                if (cudaMemcpyAsync(d_proj + off, h_in + off, cnt * sizeof(float), cudaMemcpyHostToDevice, cs) != cudaSuccess) rc = CT_ERR_CUDA;
-                cudaEventRecord(ev[c], cs);
-                cudaStreamWaitEvent(st, ev[c], 0);
+                ok(cudaMemcpyAsync(d_proj + off, h_in + off, cnt * sizeof(float), cudaMemcpyHostToDevice, cs));
+                ok(cudaEventRecord(ev, cs));
+                ok(cudaStreamWaitEvent(st, ev, 0));
                 if (rc == CT_OK) {
                     const int n = ctsf_launch_bp(g, d_proj + off, d_vol, 1, v0, 1, v1 - v0, stream, c > 0);
                     if (n < 0) rc = CT_ERR_CUDA; else launches += n;
                 }
             }
         }
-        if (!fwd && rc == CT_OK && cudaMemcpyAsync(h_out, d_vol, nvol * sizeof(float), cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = CT_ERR_CUDA;
-        if (cs) {
+        if (d_volT) ctsf_scratch_release(g, d_volT, stream);
+        if (!fwd && rc == CT_OK) ok(cudaMemcpyAsync(h_out, d_vol, nvol * sizeof(float), cudaMemcpyDeviceToHost, st));
+        if (cs && !g->host_events.empty() && g->host_events[MAX_CHUNKS]) {
             // `st` must outlive the copies of `cs` before the buffers are freed on it
-            if (start) { cudaEventRecord(start, cs); cudaStreamWaitEvent(st, start, 0); }
+            cudaEvent_t start = (cudaEvent_t)g->host_events[MAX_CHUNKS];
+            cudaEventRecord(start, cs);
+            cudaStreamWaitEvent(st, start, 0);
         }
-        cudaFreeAsync(d_vol, st);
-        cudaFreeAsync(d_proj, st);
-        d_vol = d_proj = nullptr;
-        if (cudaStreamSynchronize(st) != cudaSuccess && rc == CT_OK) rc = CT_ERR_CUDA;
-        for (int c = 0; c < n_chunks; ++c) if (ev[c]) cudaEventDestroy(ev[c]);
-        if (start) cudaEventDestroy(start);
-        if (cs) cudaStreamDestroy(cs);
     }
-    if (d_vol) cudaFreeAsync(d_vol, st);
-    if (d_proj) cudaFreeAsync(d_proj, st);
+    cudaFreeAsync(d_vol, st);
+    cudaFreeAsync(d_proj, st);
     if (cudaStreamSynchronize(st) != cudaSuccess && rc == CT_OK) rc = CT_ERR_CUDA;
-    const_cast<ct_geom *>(g)->last_launches.store(launches);
+    g->last_launches.store(launches);
     if (rc != CT_OK) cudaGetLastError();
     return rc;
 }

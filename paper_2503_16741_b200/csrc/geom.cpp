@@ -151,7 +151,7 @@ ct_status_t ctsf_build_views(const ct_geom_desc_t *d, ct_geom *g)
             // bounds over the part of the volume that projects on or near the detector
             const int np = sw ? d->ny : d->nx, nq = sw ? d->nx : d->ny, nz = is3 ? d->nz : 1;
             const int NS = 9;
-            double gp_min = 1e300, hk_max = 0, hl_max = 0;
+            double gp_min = 1e300, hk_max = 0, hl_max = 0, lpad_max = 0, zpad_max = 0;
             int used = 0;
             for (int sz = 0; sz < (is3 ? NS : 1); ++sz) for (int sq = 0; sq < NS; ++sq) for (int sp = 0; sp < NS; ++sp) {
                 double p = (np - 1) * sp / double(NS - 1), q = (nq - 1) * sq / double(NS - 1);
@@ -172,7 +172,23 @@ ct_status_t ctsf_build_views(const ct_geom_desc_t *d, ct_geom *g)
                 hk_max = std::max(hk_max, std::max(khi - kc, kc - klo));
                 if (is3) {
                     m.project(p, q, z + 0.5, k1, l1); m.project(p, q, z - 0.5, k2, l2);
-                    hl_max = std::max(hl_max, std::max(std::fabs(l1 - lc), std::fabs(l2 - lc)));
+                    const double hl_rect = std::max(std::fabs(l1 - lc), std::fabs(l2 - lc));
+                    const double rows_per_z = std::fabs(l1 - l2);                 // rows one voxel spans along z
+                    hl_max = std::max(hl_max, hl_rect);
+                    if (d->algo == CT_ALGO_SFTT) {
+                        // SF-TT (R27): the axial trapezoid's vertices are the rows of the in-plane chord's ends at z -+ 1/2
+                        const double ep = p + (sw ? ey0 : ex0), eq = q + (sw ? ex0 : ey0);
+                        const double hm = 0.5 / std::max(std::fabs(ep), std::fabs(eq));
+                        double hl_trap = 0.0;
+                        for (int sn = -1; sn <= 1; sn += 2) for (int sz = -1; sz <= 1; sz += 2) {
+                            m.project(p + sn * ep * hm, q + sn * eq * hm, z + 0.5 * sz, k1, l1);
+                            hl_trap = std::max(hl_trap, std::fabs(l1 - lc));
+                        }
+                        hl_max = std::max(hl_max, hl_trap);
+                        const double extra = std::max(0.0, hl_trap - hl_rect);
+                        lpad_max = std::max(lpad_max, extra);
+                        zpad_max = std::max(zpad_max, extra / std::max(rows_per_z, 1e-6));
+                    }
                 }
             }
             // lane stride of the forward kernel: voxels p and p + stride must project >= 1 cell apart
@@ -187,6 +203,9 @@ ct_status_t ctsf_build_views(const ct_geom_desc_t *d, ct_geom *g)
             o.lane_stride = std::max(stride, 1);
             o.ek = (float)(hk_max * 1.10 + 0.05);
             o.el = (float)(is3 ? hl_max * 1.10 + 0.05 : 0.0);
+            o.lpad = (float)(d->algo == CT_ALGO_SFTT && is3 ? lpad_max * 1.25 + 0.1 : 0.0);
+            o.zpad = (float)(d->algo == CT_ALGO_SFTT && is3 ? zpad_max * 1.25 + 0.1 : 0.0);
+            g->h_bp[i].lpad = o.lpad;                  // the backprojector's brick shadow uses the same margin
             // columns / rows one footprint can span: floor(kc+t3) - floor(kc+t0) + 1 <= 2 ek + 2
             if (2.0 * o.ek + 2.0 > 6.0 || 2.0 * o.el + 2.0 > 8.0) small_fp = 0;
             g->h_fp[i] = o;

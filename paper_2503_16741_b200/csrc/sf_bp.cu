@@ -169,7 +169,7 @@ __device__ __forceinline__ TileInfo brick_shadow(const SfView &v, const SfProble
     kmin = __shfl_sync(0xffffffffu, kmin, 0); kmax = __shfl_sync(0xffffffffu, kmax, 0);
     lmin = __shfl_sync(0xffffffffu, lmin, 0); lmax = __shfl_sync(0xffffffffu, lmax, 0);
     // margins: fp32 rounding of the corner projections, and (arc) the bulge of rows between corners
-    const float mk = 0.75f, ml = ARC ? 1.5f : 0.75f;
+    const float mk = 0.75f, ml = (ARC ? 1.5f : 0.75f) + v.lpad;
     TileInfo t;
     // TMA: the innermost box coordinate must be 16-byte aligned (measured on B200: an odd start
     // coordinate raises 'illegal instruction'), so the tile origin is rounded down to 4 cells
@@ -195,7 +195,7 @@ __device__ __forceinline__ float gather_tile(uint32_t tile_a, const SfTrans &T, 
     for (int lb = l_lo; lb <= l_hi; lb += LM) {
         // rows past l_hi get weight 0 by themselves (x >= thi), rows past the tile read the zero pad rows
         float f2[LM];
-        sf_F2_run<LM>(A, (float)lb, f2);
+        sf_F2_run<LM, MODEL>(A, (float)lb, f2);
         uint32_t ra = tile_a + 4u * (unsigned)((lb - tl0) * TW + (k_lo - tk0));
         float xi = (float)k_lo - T.kc;
         float g0 = sf_G<MODEL>(T, xi);
@@ -221,7 +221,7 @@ __device__ __forceinline__ float gather_tile_ptr(const float *__restrict__ tile,
     float sum = 0.0f;
     for (int lb = l_lo; lb <= l_hi; lb += LM) {
         float f2[LM];
-        sf_F2_run<LM>(A, (float)lb, f2);
+        sf_F2_run<LM, MODEL>(A, (float)lb, f2);
         const float *row = tile + (lb - tl0) * TW + (k_lo - tk0);
         float xi = (float)k_lo - T.kc;
         float g0 = sf_G<MODEL>(T, xi);
@@ -391,13 +391,13 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
                             if (k_lo > k_hi) continue;
                             const float c = fmaf(z, v.cz, c_col);
                             SfAxial A;
-                            sf_axial<ARC>(v, a, b, c, inv_a, A);
+                            sf_axial<ARC, MODEL>(v, a, b, c, inv_a, A, p, q);
                             const int l_lo = max(max(0, tl0), (int)floorf(A.lc + A.tlo));
                             const int l_hi = min(min(pr.nv - 1, tl0 + TH - 1), (int)floorf(A.lc + A.thi));
                             if (l_lo > l_hi) continue;
                             float amp, sum;
                             if (UNT) {
-                                amp = RECON ? sf_recon_weight_s<ARC>(v, sumF1, A.thi - A.tlo, a, b)
+                                amp = RECON ? sf_recon_weight_s<ARC>(v, sumF1, sf_axial_sum<MODEL>(A), a, b)
                                             : sf_amplitude(v, a, b, c, p, q);
                                 const int K = k_hi - k_lo + 1;
                                 if (K <= BKR) {
@@ -408,7 +408,7 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
                                     sum = gather_tile_ptr<MODEL>(tile, T2, A, k_lo, k_hi, l_lo, l_hi, tk0, tl0);
                                 }
                             } else {
-                                amp = RECON ? sf_recon_weight<ARC>(v, T, A.thi - A.tlo, a, b)
+                                amp = RECON ? sf_recon_weight<ARC>(v, T, sf_axial_sum<MODEL>(A), a, b)
                                             : sf_amplitude(v, a, b, c, p, q);
                                 sum = gather_tile<MODEL>(tile_a, T, A, k_lo, k_hi, l_lo, l_hi, tk0, tl0);
                             }
@@ -669,26 +669,27 @@ int launch_brick(const ct_geom *g, const float *d_proj, float *d_vol, int batch,
     memset(&tmap, 0, sizeof tmap);
     int use_tma = 0;
     EncodeTiledFn enc = get_encode();
-    const char *dbg = getenv("CTSF_BP_TMA");
-    if (enc && !(dbg && dbg[0] == '0') && vc > 0 && pr.nu % 4 == 0 && ((uintptr_t)d_proj & 15u) == 0) {
+    const int dbg_tma = g_ctsf_debug.bp_tma;            // testing aid: -1 default, 0 cp.async only, 1..3 partial TMA use
+    if (enc && dbg_tma != 0 && vc > 0 && pr.nu % 4 == 0 && ((uintptr_t)d_proj & 15u) == 0) {
         cuuint64_t dims[3] = {(cuuint64_t)pr.nu, (cuuint64_t)pr.nv, (cuuint64_t)vc * batch};
         cuuint64_t strides[2] = {(cuuint64_t)pr.nu * 4, (cuuint64_t)pr.nu * pr.nv * 4};
         cuuint32_t box[3] = {TW, TH, 1}, es[3] = {1, 1, 1};
         if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)d_proj, dims, strides, box, es,
                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS)
-            use_tma = (dbg && dbg[0] >= '1' && dbg[0] <= '3') ? dbg[0] - '0' : 3;
+            use_tma = (dbg_tma >= 1 && dbg_tma <= 3) ? dbg_tma : 3;
     }
     const size_t smem = (size_t)(2 * TILE_FLOATS + BZ * BRICK_THREADS) * sizeof(float);
     const size_t smem2 = (size_t)(BP2_STAGES * TILE_FLOATS + BZ * BRICK_THREADS) * sizeof(float);
     // untilted frames with small footprints (host bound): F1 weights live in registers along the z-run
-    // (testing aids: CTSF_BP_NOHOIST / CTSF_BP_FORCEHOIST, as for the forward kernel)
-    const bool hoist = !getenv("CTSF_BP_NOHOIST") &&
-                       (g->fp_hoist_ok || (g->all_untilted && getenv("CTSF_BP_FORCEHOIST")));
-    // general frames: the packed two-voxel kernel (needs the TMA path); CTSF_BP_SCALAR=1 (testing aid) keeps the
+    // (testing aids bp_nohoist / bp_forcehoist of CtsfDebug, as for the forward kernel)
+    const bool hoist = !g_ctsf_debug.bp_nohoist &&
+                       (g->fp_hoist_ok || (g->all_untilted && g_ctsf_debug.bp_forcehoist)) && g->model != 2;
+    // general frames: the packed two-voxel kernel (needs the TMA path); the testing aid bp_scalar keeps the
     // one-voxel-per-thread kernel
-    const bool packed = !hoist && use_tma == 3 && !getenv("CTSF_BP_SCALAR");
-    auto kern = g->model == 1
+    const bool packed = !hoist && use_tma == 3 && !g_ctsf_debug.bp_scalar && g->model != 2;
+    auto kern = g->model == 2 ? (recon ? bp_brick_kernel<ARC, 1, 0, 2> : bp_brick_kernel<ARC, 0, 0, 2>)
+        : g->model == 1
         ? (hoist ? (recon ? bp_brick_kernel<ARC, 1, 1, 1> : bp_brick_kernel<ARC, 0, 1, 1>)
                  : (recon ? bp_brick_kernel<ARC, 1, 0, 1> : bp_brick_kernel<ARC, 0, 0, 1>))
         : (hoist ? (recon ? bp_brick_kernel<ARC, 1, 1, 0> : bp_brick_kernel<ARC, 0, 1, 0>)
@@ -705,8 +706,7 @@ int launch_brick(const ct_geom *g, const float *d_proj, float *d_vol, int batch,
     const size_t view_bytes = (size_t)pr.nu * pr.nv * sizeof(float) * batch;
     int chunk = (int)((96u << 20) / (view_bytes ? view_bytes : 1));
     if (chunk < 8) chunk = 8;
-    const char *cdbg = getenv("CTSF_BP_CHUNK");
-    if (cdbg && atoi(cdbg) > 0) chunk = atoi(cdbg);
+    if (g_ctsf_debug.bp_chunk > 0) chunk = g_ctsf_debug.bp_chunk;
     for (int j_lo = 0; j_lo < vc || (vc == 0 && j_lo == 0); j_lo += chunk) {
         const int j_hi = j_lo + chunk < vc ? j_lo + chunk : vc;
         for (int b0 = 0; b0 < batch;) {
@@ -737,7 +737,7 @@ void launch_pixel(const ct_geom *g, const float *d_proj, float *d_vol, int b0, i
     const size_t pbs = (size_t)vc * pr.nu, vbs = (size_t)pr.nx * pr.ny;
     dim3 block(16, 8, 1);
     dim3 grid((pr.nx + block.x - 1) / block.x, (pr.ny + block.y - 1) / block.y, groups);
-    auto kern = g->model == 1 ? (recon ? bp_pixel_kernel<ARC, NB, 1, 1> : bp_pixel_kernel<ARC, NB, 0, 1>)
+    auto kern = g->model == 1 ? (recon ? bp_pixel_kernel<ARC, NB, 1, 1> : bp_pixel_kernel<ARC, NB, 0, 1>)     // 2-D: SF-TT == SF-TR
                               : (recon ? bp_pixel_kernel<ARC, NB, 1, 0> : bp_pixel_kernel<ARC, NB, 0, 0>);
     kern<<<grid, block, 0, st>>>(pr, g->d_bp, d_proj + (size_t)b0 * pbs, d_vol + (size_t)b0 * vbs,
                                  vb, vs, vc, (unsigned)pbs, (unsigned)vbs);

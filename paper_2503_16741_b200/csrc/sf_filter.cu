@@ -21,7 +21,7 @@ constexpr int FJ = 8;              // outputs per thread (register tile of the T
 template <int ARC>
 __global__ void __launch_bounds__(FLT_THREADS)
 fbp_filter_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ proj,
-                  float *__restrict__ out, int view_begin, int view_stride, int view_count, double du, double dv)
+                  float *__restrict__ out, int view_begin, int view_stride, int view_count, double du, double dv, double scale)
 {
     extern __shared__ double sm[];
     double *pw = sm, *h = sm + pr.nu;             // h is stored padded: entry n at HP(n) = n + n/16
@@ -91,7 +91,7 @@ fbp_filter_kernel(SfProblem pr, const SfView *__restrict__ views, const float *_
 #pragma unroll
         for (int j = 0; j < FJ; ++j) {
             const int k = kb + 2 * j;
-            if (k < pr.nu) q[k] = (float)(du * fma(pw[k], h[0], acc[j]));      // HP(0) = 0
+            if (k < pr.nu) q[k] = (float)(scale * du * fma(pw[k], h[0], acc[j]));      // HP(0) = 0
         }
     }
 }
@@ -99,7 +99,7 @@ fbp_filter_kernel(SfProblem pr, const SfView *__restrict__ views, const float *_
 }  // namespace
 
 int ctsf_launch_filter(const ct_geom *g, const float *d_proj, float *d_out, int batch,
-                       int view_begin, int view_stride, int view_count, void *stream)
+                       int view_begin, int view_stride, int view_count, void *stream, double scale)
 {
     const SfProblem &pr = g->prob;
     const long rows = (long)batch * view_count * pr.nv;
@@ -116,7 +116,7 @@ int ctsf_launch_filter(const ct_geom *g, const float *d_proj, float *d_out, int 
         // a chunk starts at a whole number of (batch, view) rows only when r0 == 0; larger problems do not occur
         kern<<<dim3((unsigned)n, 1, 1), FLT_THREADS, smem, (cudaStream_t)stream>>>(
             pr, g->d_bp, d_proj + (size_t)r0 * pr.nu, d_out + (size_t)r0 * pr.nu, view_begin, view_stride, view_count,
-            g->du, g->dv);
+            g->du, g->dv, scale);
         ++launches;
     }
     return cudaGetLastError() == cudaSuccess ? launches : -1;

@@ -163,8 +163,10 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
 #pragma unroll
     for (int s_ = 1; s_ < 8; s_ <<= 1) slope = fmaxf(slope, __shfl_xor_sync(FULL, slope, s_));
     slope = __shfl_sync(FULL, slope, 0);
-    const float hp = 0.6f + 0.5f * fminf(slope, 4.0f) + region_pad;
-    const float hz = (ARC ? 1.5f : 1.1f) + region_pad;            // 1/2 voxel + 1/2 (rounded shear shift) + margin (arc: bulge)
+    // hp = 1/2 + 1/2 |dp/dq| is exact (+ 0.1 margin).  Beyond slope 8 (tile-edge rays within 7 degrees of the slab:
+    // fans wider than ~75 degrees, or very anisotropic pitches) the whole in-slab range is swept instead
+    const float hp = slope > 8.0f ? 1e9f : 0.6f + 0.5f * slope + region_pad;
+    const float hz = (ARC ? 1.5f : 1.1f) + region_pad + (MODEL == 2 ? v.zpad : 0.0f);            // 1/2 voxel + 1/2 (rounded shear shift) + margin (arc: bulge)
     __syncwarp();
 
     const int np = v.swap_xy ? pr.ny : pr.nx, nq = v.swap_xy ? pr.nx : pr.ny, nz = pr.nz;
@@ -368,7 +370,7 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
                 SfAxial A;
                 int l_lo = 0, l_hi = 0;
                 if (DIM == 3) {
-                    sf_axial<ARC>(v, a, b, c, inv_a, A);
+                    sf_axial<ARC, MODEL>(v, a, b, c, inv_a, A, p, q);
                     l_lo = max(l0, (int)floorf(A.lc + A.tlo));
                     l_hi = min(l_top, (int)floorf(A.lc + A.thi));
                     if (!__any_sync(FULL, act && l_lo <= l_hi)) continue;
@@ -410,8 +412,8 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
                     for (int lb = 0; lb < Lmax; lb += 2 * FLM) {
                         float f2[2 * FLM];
                         if (DIM == 3) {
-                            if (Lmax > lb + FLM) sf_F2_run<2 * FLM>(A, (float)(l_lo + lb), f2);
-                            else                 sf_F2_run<FLM>(A, (float)(l_lo + lb), f2);
+                            if (Lmax > lb + FLM) sf_F2_run<2 * FLM, MODEL>(A, (float)(l_lo + lb), f2);
+                            else                 sf_F2_run<FLM, MODEL>(A, (float)(l_lo + lb), f2);
                         }
                         float xi = xi0, g0 = sf_G<MODEL>(T, xi0);
                         uint32_t ca = smem_addr(base + lb * FTK);      // this lane's cell of round 0
@@ -439,6 +441,7 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
                             CTSF_ROUNDS(_Pragma("unroll") for (int bb = 0; bb < NB; ++bb)
                                             sts_f32(ca + bb * FTK * 4, fmaf(f1, xv[bb], lds_f32(ca + bb * FTK * 4)));)
                         }
+#undef CTSF_ROUNDS
 #undef CTSF_ROUNDS
                     }
                 }
@@ -469,24 +472,25 @@ void launch_fp(const ct_geom *g, const float *d_vol, const float *d_volT, float 
     const size_t vbs = (size_t)pr.nx * pr.ny * pr.nz, pbs = (size_t)vc * pr.nv * pr.nu;
     constexpr int ROWS = DIM == 3 ? FTL + FLM : NB;
     const size_t smem = (size_t)FPW * ROWS * FTK * sizeof(float);
-    // testing aids: CTSF_FP_NOHOIST=1 never uses the untilted fast path; CTSF_FP_FORCEHOIST=1 uses it for every
+    // testing aids (CtsfDebug): fp_nohoist never uses the untilted fast path; fp_forcehoist uses it for every
     // untilted 3-D geometry, also when footprints exceed its register windows (exercises its overflow branch)
-    const bool hoist = DIM == 3 && !getenv("CTSF_FP_NOHOIST") &&
-                       (g->fp_hoist_ok || (g->all_untilted && getenv("CTSF_FP_FORCEHOIST")));
-    auto kern = g->model == 1
+    const bool hoist = DIM == 3 && !g_ctsf_debug.fp_nohoist &&
+                       (g->fp_hoist_ok || (g->all_untilted && g_ctsf_debug.fp_forcehoist)) && g->model != 2;
+    // SF-TT (model 2) differs from SF-TR in the axial factor only: 2-D geometries run the SF-TR instantiation
+    auto kern = (g->model == 2 && DIM == 3) ? fp_band_kernel<DIM, ARC, NB, 0, DIM == 3 ? 2 : 0>
+        : g->model == 1
         ? (hoist ? fp_band_kernel<DIM, ARC, NB, DIM == 3 ? 1 : 0, 1> : fp_band_kernel<DIM, ARC, NB, 0, 1>)
         : (hoist ? fp_band_kernel<DIM, ARC, NB, DIM == 3 ? 1 : 0, 0> : fp_band_kernel<DIM, ARC, NB, 0, 0>);
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const long n_items = (long)tiles_k * bands_l * ((vc + FVG - 1) / FVG) * FVG;
-    // testing aid: CTSF_FP_PAD=<voxels> widens the swept voxel region; the result must not change beyond
+    // testing aid: fp_pad = <voxels> widens the swept voxel region; the result must not change beyond
     // summation order (tests/test_gpu_fullsize.py uses it to prove that the tight region misses nothing)
-    const char *pad_env = getenv("CTSF_FP_PAD");
-    const float region_pad = pad_env ? (float)atof(pad_env) : 0.0f;
+    const float region_pad = g_ctsf_debug.fp_pad;
     dim3 grid((unsigned)((n_items + FPW - 1) / FPW), groups, 1);
     kern<<<grid, 32 * FPW, smem, st>>>(pr, g->d_fp, d_vol + (size_t)b0 * vbs,
                                        d_volT ? d_volT + (size_t)b0 * vbs : nullptr,
                                        d_proj + (size_t)b0 * pbs, vb, vs, tiles_k, bands_l, (int)n_items, vc, vbs, pbs, region_pad,
-                                       getenv("CTSF_FP_SERIAL") ? 1 : 0);   // testing aid: take the lane-serial branch
+                                       g_ctsf_debug.fp_serial ? 1 : 0);   // testing aid: take the lane-serial branch
 }
 
 template <int DIM, int ARC>
@@ -524,34 +528,50 @@ int launch_fp_batches(const ct_geom *g, const float *d_vol, const float *d_volT,
 
 }  // namespace
 
+bool ctsf_fp_needs_transpose(const ct_geom *g, int view_begin, int view_stride, int view_count)
+{
+    for (int j = 0; j < view_count; ++j)
+        if (g->h_fp[view_begin + (size_t)j * view_stride].swap_xy != 0) return true;
+    return false;
+}
+
+int ctsf_fp_transpose(const ct_geom *g, const float *d_vol, float *d_volT, int batch, void *stream)
+{
+    const SfProblem &pr = g->prob;
+    int launches = 0;
+    dim3 grid((pr.nx + 31) / 32, (pr.ny + 31) / 32, 1), block(32, 8);
+    const long slices = (long)batch * pr.nz;                 // one launch per chunk of <= 65535 slices
+    for (long s0 = 0; s0 < slices; s0 += 65535) {
+        grid.z = (unsigned)((slices - s0) < 65535 ? (slices - s0) : 65535);
+        transpose_xy_kernel<<<grid, block, 0, (cudaStream_t)stream>>>(d_vol + (size_t)s0 * pr.nx * pr.ny,
+                                                                      d_volT + (size_t)s0 * pr.nx * pr.ny, pr.nx, pr.ny);
+        ++launches;
+    }
+    return cudaGetLastError() == cudaSuccess ? launches : -1;
+}
+
 int ctsf_launch_fp(const ct_geom *g, const float *d_vol, float *d_proj, int batch,
-                   int view_begin, int view_stride, int view_count, void *stream)
+                   int view_begin, int view_stride, int view_count, void *stream, const float *d_volT_in)
 {
     cudaStream_t st = (cudaStream_t)stream;
     const SfProblem &pr = g->prob;
     int launches = 0;
-    float *d_volT = nullptr;
-    bool need_T = false;
-    for (int j = 0; j < view_count && !need_T; ++j) need_T = g->h_fp[view_begin + (size_t)j * view_stride].swap_xy != 0;
-    if (need_T) {
+    const float *d_volT = d_volT_in;
+    float *scratch = nullptr;
+    if (!d_volT && ctsf_fp_needs_transpose(g, view_begin, view_stride, view_count)) {
         const size_t n = (size_t)batch * pr.nx * pr.ny * pr.nz;
-        d_volT = (float *)ctsf_alloc_async(n * sizeof(float), st);
-        if (!d_volT) return -1;
-        dim3 grid((pr.nx + 31) / 32, (pr.ny + 31) / 32, 1), block(32, 8);
-        // one launch per chunk of <= 65535 slices
-        const long slices = (long)batch * pr.nz;
-        for (long s0 = 0; s0 < slices; s0 += 65535) {
-            grid.z = (unsigned)((slices - s0) < 65535 ? (slices - s0) : 65535);
-            transpose_xy_kernel<<<grid, block, 0, st>>>(d_vol + (size_t)s0 * pr.nx * pr.ny,
-                                                        d_volT + (size_t)s0 * pr.nx * pr.ny, pr.nx, pr.ny);
-            ++launches;
-        }
+        scratch = (float *)ctsf_scratch_acquire(g, n * sizeof(float), stream);
+        if (!scratch) return -1;
+        const int nt = ctsf_fp_transpose(g, d_vol, scratch, batch, stream);
+        if (nt < 0) { ctsf_scratch_release(g, scratch, stream); return -1; }
+        launches += nt;
+        d_volT = scratch;
     }
     const int arc = pr.det_type;
     if (pr.dim == 2) launches += arc ? launch_fp_batches<2, 1>(g, d_vol, d_volT, d_proj, batch, view_begin, view_stride, view_count, st)
                                      : launch_fp_batches<2, 0>(g, d_vol, d_volT, d_proj, batch, view_begin, view_stride, view_count, st);
     else             launches += arc ? launch_fp_batches<3, 1>(g, d_vol, d_volT, d_proj, batch, view_begin, view_stride, view_count, st)
                                      : launch_fp_batches<3, 0>(g, d_vol, d_volT, d_proj, batch, view_begin, view_stride, view_count, st);
-    ctsf_free_async(d_volT, st);
+    if (scratch) ctsf_scratch_release(g, scratch, stream);
     return cudaGetLastError() == cudaSuccess ? launches : -1;
 }

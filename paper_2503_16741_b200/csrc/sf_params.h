@@ -37,7 +37,8 @@ struct SfView {
     float ek, el;              // max footprint half extent (cells / rows) over the view, x1.1: host-side bound on K, L
     int32_t lane_stride;       // voxels p, p + lane_stride project >= 1 cell apart (conflict-free rounds)
     float recon_dR;            // recon mode (reading R23): d * R, d = distance source -> rotation centre (world origin)
-    int32_t pad1, pad2;
+    float lpad;                // SF-TT (MODEL 2): rows the axial trapezoid reaches beyond the rectangle (brick shadow margin)
+    float zpad;                // ... the same in voxels along z (forward kernel's region halo)
 };
 
 struct SfProblem {

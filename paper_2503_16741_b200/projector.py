@@ -18,7 +18,7 @@ class Geometry:
         torch.cuda.current_device()          # make sure a context exists before libctsf allocates
         torch.zeros(1, device="cuda")
         self.handle = B.ct_geom_create(g)
-        self.algo = {0: "SF", 1: "DD"}.get(g.get("algo", "SF"), g.get("algo", "SF"))
+        self.algo = {0: "SF", 1: "DD", 2: "SF-TT"}.get(g.get("algo", "SF"), g.get("algo", "SF"))
         self.dim = int(g["dim"])
         self.vol_shape = (int(g.get("nz", 1)), int(g["ny"]), int(g["nx"]))
         self.n_views = len(g["src"])
@@ -45,67 +45,120 @@ class Geometry:
     def fp(self, vol, views=None, out=None):
         """vol [..., nz, ny, nx] -> proj [..., n_sel, nv, nu]."""
         vb, vs, vc = self._views(views)
-        lead, batch, vol = _prep(vol, self.vol_shape)
-        if out is None:
-            out = torch.empty((batch, vc) + self.det_shape, device=vol.device, dtype=torch.float32)
+        lead, batch, vol = _prep(vol, self.vol_shape, -3 if self.dim == 2 else None)
+        out = _out(out, (batch, vc) + self.det_shape, vol.device)
         B.ct_fp_sf_views(self.handle, vol.data_ptr(), out.data_ptr(), batch, vb, vs, vc,
                          torch.cuda.current_stream(vol.device).cuda_stream)
-        return out.view(lead + (vc,) + self.det_shape)
+        return out.view(lead + self._tail((vc,) + self.det_shape, -2, vol))
 
     def bp(self, proj, views=None, out=None):
         """proj [..., n_sel, nv, nu] -> vol [..., nz, ny, nx]."""
         vb, vs, vc = self._views(views)
-        lead, batch, proj = _prep(proj, (vc,) + self.det_shape)
-        if out is None:
-            out = torch.empty((batch,) + self.vol_shape, device=proj.device, dtype=torch.float32)
+        lead, batch, proj = _prep(proj, (vc,) + self.det_shape, -2 if self.dim == 2 else None)
+        out = _out(out, (batch,) + self.vol_shape, proj.device)
         B.ct_bp_sf_views(self.handle, proj.data_ptr(), out.data_ptr(), batch, vb, vs, vc,
                          torch.cuda.current_stream(proj.device).cuda_stream)
-        return out.view(lead + self.vol_shape)
+        return out.view(lead + self._tail(self.vol_shape, -3, proj))
 
     # ---- recon mode (PAPER.md:103, 68; DESIGN.md readings R23, R24) --------------------------------
     def fbp_filter(self, proj, views=None, out=None):
         """Cosine pre-weight + discrete ramp filter along the channels; proj [..., n_sel, nv, nu] -> same shape."""
         vb, vs, vc = self._views(views)
-        lead, batch, proj = _prep(proj, (vc,) + self.det_shape)
-        if out is None:
-            out = torch.empty_like(proj)
+        lead, batch, proj = _prep(proj, (vc,) + self.det_shape, -2 if self.dim == 2 else None)
+        out = _out(out, tuple(proj.shape), proj.device)
         B.ct_fbp_filter_views(self.handle, proj.data_ptr(), out.data_ptr(), batch, vb, vs, vc,
                               torch.cuda.current_stream(proj.device).cuda_stream)
-        return out.view(lead + (vc,) + self.det_shape)
+        return out.view(lead + self._tail((vc,) + self.det_shape, -2, proj))
 
     def bp_recon(self, proj, views=None, out=None):
         """Recon-mode backprojection (normalised footprints x depth weight); proj [..., n_sel, nv, nu] -> volume."""
         vb, vs, vc = self._views(views)
-        lead, batch, proj = _prep(proj, (vc,) + self.det_shape)
-        if out is None:
-            out = torch.empty((batch,) + self.vol_shape, device=proj.device, dtype=torch.float32)
+        lead, batch, proj = _prep(proj, (vc,) + self.det_shape, -2 if self.dim == 2 else None)
+        out = _out(out, (batch,) + self.vol_shape, proj.device)
         B.ct_bp_sf_recon_views(self.handle, proj.data_ptr(), out.data_ptr(), batch, vb, vs, vc,
                                torch.cuda.current_stream(proj.device).cuda_stream)
-        return out.view(lead + self.vol_shape)
+        return out.view(lead + self._tail(self.vol_shape, -3, proj))
 
-    def fbp(self, proj):
-        """Filtered backprojection of N equi-angular views over 360 degrees: (pi / N) B(filter(p))."""
-        import math
-        return self.bp_recon(self.fbp_filter(proj)).mul_(math.pi / self.n_views)
+    def fbp(self, proj, out=None):
+        """Filtered backprojection of N equi-angular views over 360 degrees: (pi / N) B(filter(p)) (ct_fbp_sf)."""
+        lead, batch, proj = _prep(proj, (self.n_views,) + self.det_shape, -2 if self.dim == 2 else None)
+        out = _out(out, (batch,) + self.vol_shape, proj.device)
+        work = torch.empty_like(proj)
+        B.ct_fbp_sf(self.handle, proj.data_ptr(), work.data_ptr(), out.data_ptr(), batch,
+                    torch.cuda.current_stream(proj.device).cuda_stream)
+        return out.view(lead + self._tail(self.vol_shape, -3, proj))
+
+    def _tail(self, tail, unit_axis, like):
+        """Output tail shape: 2-D inputs given without their unit axis ([..., ny, nx] / [..., views, nu], the paper's
+        own usage) get outputs without theirs too."""
+        tail = tuple(tail)
+        if self.dim == 2 and getattr(like, "_ctsf_squeezed", False):
+            i = len(tail) + unit_axis
+            return tail[:i] + tail[i + 1:]
+        return tail
 
     def last_launch_count(self):
         return B.ct_last_launch_count(self.handle)
 
+    # ---- view-sharded operators (SURVEY 8(e) item 2; DESIGN.md "Multi-GPU") -------------------------------
+    def fp_sharded(self, vol, rank, world_size, out=None):
+        """This rank's views of A x (volume replicated): returns ((view_begin, view_stride, view_count), projections)."""
+        from .geometry import shard_views
+        sub = shard_views(self.n_views, world_size, rank)
+        return sub, self.fp(vol, views=sub, out=out)
 
-def _prep(t, tail):
+    def bp_sharded(self, proj_shard, rank, world_size, group=None, out=None):
+        """A^T y with the views sharded over the ranks of `group`: every rank backprojects its own shard
+        (ct_bp_sf_views) into a full-size partial volume; ONE sum all-reduce (NCCL) makes them the result."""
+        import torch.distributed as dist
+        from .geometry import shard_views
+        sub = shard_views(self.n_views, world_size, rank)
+        x = self.bp(proj_shard, views=sub, out=out)
+        if world_size > 1:
+            dist.all_reduce(x, op=dist.ReduceOp.SUM, group=group)
+        return x
+
+
+def _prep(t, tail, unit_axis=None):
+    """Contiguous fp32 view [batch, *tail] of a CUDA tensor whose trailing dims are `tail`.  unit_axis (2-D geometries):
+    index in `tail` of the unit z / row axis, which may be missing: [..., ny, nx] and [..., views, nu] are accepted."""
     if not t.is_cuda:
         raise RuntimeError("ctsf operators take CUDA tensors (no CPU fallback)")
+    if t.dtype != torch.float32:
+        raise TypeError("ctsf operators compute in float32; got %s (cast explicitly)" % t.dtype)
+    tail = tuple(tail)
     nd = len(tail)
-    if tuple(t.shape[-nd:]) != tuple(tail):
-        raise ValueError("expected trailing shape %s, got %s" % (tail, tuple(t.shape)))
+    squeezed = False
+    if tuple(t.shape[-nd:]) != tail:
+        i = nd + unit_axis if unit_axis is not None else None
+        short = tail[:i] + tail[i + 1:] if i is not None else None
+        if short is not None and tail[i] == 1 and tuple(t.shape[-(nd - 1):]) == short:
+            t = t.unsqueeze(t.dim() - (nd - 1) + i)
+            squeezed = True
+        else:
+            raise ValueError("expected trailing shape %s, got %s" % (tail, tuple(t.shape)))
     lead = tuple(t.shape[:-nd])
-    t = t.detach().to(torch.float32).contiguous()
+    t = t.detach().contiguous()
     batch = 1
     for s in lead:
         batch *= s
     if batch < 1:
         raise ValueError("empty batch")
-    return lead, batch, t.view((batch,) + tuple(tail))
+    t = t.view((batch,) + tail)
+    t._ctsf_squeezed = squeezed
+    return lead, batch, t
+
+
+def _out(out, shape, device):
+    """A fresh output, or the caller's after checking what the library cannot: dtype, device, size, contiguity."""
+    if out is None:
+        return torch.empty(shape, device=device, dtype=torch.float32)
+    n = 1
+    for s in shape:
+        n *= s
+    if out.dtype != torch.float32 or out.device != device or out.numel() != n or not out.is_contiguous():
+        raise ValueError("out= must be a contiguous float32 tensor of %d elements on %s" % (n, device))
+    return out
 
 
 class FP(torch.autograd.Function):
@@ -136,14 +189,14 @@ class BP(torch.autograd.Function):
 
 class Projector(torch.nn.Module):
     """`A = Projector(geom, 'proj', 'SF', 'forward'); sino = A(img)` (PAPER.md:118-122).
-    Algorithm 'SF' (separable footprint) or 'DD' (distance-driven); mode 'proj' (matched pair, differentiable) or 'recon' (FBP backprojection of
+    Algorithm 'SF' (separable footprint, SF-TR), 'SF-TT' (trapezoid axial factor) or 'DD' (distance-driven); mode 'proj' (matched pair, differentiable) or 'recon' (FBP backprojection of
     PAPER.md:103, direction 'backward' only); direction is 'forward' or 'backward'.
     `subset=(view_begin, view_stride, view_count)` restricts to an ordered subset."""
 
     def __init__(self, geom, mode="proj", algo="SF", direction="forward"):
         super().__init__()
-        if mode not in ("proj", "recon") or algo not in ("SF", "DD"):
-            raise NotImplementedError("algo 'SF' or 'DD' with mode 'proj' or 'recon' is built (see DESIGN.md)")
+        if mode not in ("proj", "recon") or algo not in ("SF", "DD", "SF-TT"):
+            raise NotImplementedError("algo 'SF', 'SF-TT' or 'DD' with mode 'proj' or 'recon' is built (see DESIGN.md)")
         if direction not in ("forward", "backward"):
             raise ValueError(direction)
         if mode == "recon" and direction != "backward":

@@ -24,3 +24,15 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+@pytest.fixture(autouse=True)
+def _reset_ctsf_debug_switches(request):
+    """The library's testing switches (binding.debug_set) never leak from one GPU test into the next."""
+    yield
+    if "gpu" in request.keywords:
+        try:
+            from paper_2503_16741_b200 import binding
+            binding.debug_set("reset")
+        except Exception:
+            pass

@@ -73,3 +73,36 @@ def test_dd_full_size_config4_sampled():
     assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= 1e-5
     assert np.abs(got - ref).max() <= 1e-4 * np.abs(ref).max()
     A.geom.close()
+
+
+def test_dd_face_tie_on_the_diagonal_views():
+    """when |e_x|/dx == |e_y|/dy exactly (voxels on the volume's diagonals in views at 45, 135, 225
+    and 315 degrees) the face choice is a tie, which reading R26 gives to the y axis.  Forward views that read the
+    transposed volume see p = y, so their comparison must flip, or A stops being the transpose of A^T on those
+    voxels.  Which side an exact tie falls on is decided by rounding (fp32 here, float64 in the oracle), so both
+    answers are valid there: the GPU pair is checked for adjointness ON the diagonal views (this is what the tie
+    rule protects) and against the oracle on the same orbit turned by 0.01 rad (no ties)."""
+    import math
+    from paper_2503_16741_b200.projector import Geometry
+    for n_side in (32, 33):
+        for turn, parity in ((0.0, False), (0.01, True)):
+            theta = 2.0 * math.pi * np.arange(8) / 8 + turn
+            src, dc, u, v = W.trajectory(8, 300.0, 600.0, "flat", theta)
+            g = dict(dim=2, nx=n_side, ny=n_side, nz=1, dx=1.0, dy=1.0, dz=1.0, ox=0.0, oy=0.0, oz=0.0, nu=96, nv=1,
+                     du=1.2, dv=1.0, det_type="flat", src=src, det_center=dc, det_u=u, det_v=v, algo="DD")
+            rng = np.random.default_rng(5 + n_side)
+            x = rng.uniform(0.5, 1.5, (1, 1, n_side, n_side)).astype(np.float32)
+            geom = Geometry(g)
+            xd = torch.from_numpy(x).cuda()
+            y = geom.fp(xd)
+            yr = torch.from_numpy(rng.uniform(0.5, 1.5, tuple(y.shape)).astype(np.float32)).cuda()
+            lhs = torch.sum(y.double() * yr.double()).item()
+            rhs = torch.sum(xd.double() * geom.bp(yr).double()).item()
+            assert abs(lhs - rhs) <= 2e-6 * abs(lhs), (n_side, turn, lhs, rhs)
+            if parity:
+                o = Oracle(g)
+                y_ref = o.fp(x)
+                _check(y, y_ref, "DD A, near-diagonal views, n = %d" % n_side)
+                y32 = y_ref.astype(np.float32)
+                _check(geom.bp(torch.from_numpy(y32).cuda()), o.bp(y32), "DD A^T, near-diagonal views, n = %d" % n_side)
+            geom.close()

@@ -10,6 +10,7 @@ import pytest
 torch = pytest.importorskip("torch")
 
 from oracle.sf_oracle import Oracle
+from paper_2503_16741_b200 import binding as B
 from paper_2503_16741_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
@@ -50,7 +51,7 @@ def test_parity_full_size_sampled(index):
                     rng.integers(0, c["nz"], N_VOX[index])], axis=1)
     ijk[0] = (0, 0, 0)
     ijk[1] = (c["nx"] - 1, c["ny"] - 1, c["nz"] - 1)
-    for b in range(min(c["batch"], 2)):
+    for b in range(c["batch"]):                     # all 16 images of config 5
         ref = o.bp_voxels(p[b], ijk)
         got = xb[b, ijk[:, 2], ijk[:, 1], ijk[:, 0]].double().cpu().numpy()
         rel = np.linalg.norm(got - ref) / np.linalg.norm(ref)
@@ -63,7 +64,7 @@ def test_parity_full_size_sampled(index):
 @pytest.mark.parametrize("index", [4, 3, 2])
 def test_forward_region_is_conservative(index, algo, monkeypatch):
     """The forward kernel sweeps, per slab, only the voxels its tile's frustum can touch (exact half-voxel halo).
-    Property that holds at any size: widening that region by a whole voxel (CTSF_FP_PAD) may only change the
+    Property that holds at any size: widening that region by a whole voxel (debug switch fp_pad) may only change the
     summation order.  Checked on EVERY cell of every view of the full-size operator (a missed voxel would
     shift a cell by ~1e-3 of its value)."""
     from paper_2503_16741_b200.projector import Geometry
@@ -74,13 +75,13 @@ def test_forward_region_is_conservative(index, algo, monkeypatch):
     rng = np.random.default_rng(77 + index)
     x = torch.from_numpy(rng.uniform(0.5, 1.5, (1, c["nz"], c["ny"], c["nx"])).astype(np.float32)).cuda()
     geom = Geometry(g)
-    monkeypatch.delenv("CTSF_FP_PAD", raising=False)
+    B.debug_set("fp_pad", 0)
     y_tight = geom.fp(x)
     torch.cuda.synchronize()
-    monkeypatch.setenv("CTSF_FP_PAD", "1.0")
+    B.debug_set("fp_pad", 1.0)
     y_wide = geom.fp(x)
     torch.cuda.synchronize()
-    monkeypatch.delenv("CTSF_FP_PAD")
+    B.debug_set("fp_pad", 0)
     diff = (y_tight - y_wide).abs().max().item()
     assert diff <= 3e-6 * y_wide.abs().max().item(), diff
     geom.close()

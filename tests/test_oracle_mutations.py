@@ -34,7 +34,7 @@ MUTATIONS = {
         "double norm = sqrt(e[0]*e[0] + e[1]*e[1]);",
         [(T3.test_tilted_frame_config4_shape, {})]),
     "axial_ends_at_0p45_dz": (
-        "double Pm[3] = { Pc[0], Pc[1], Pc[2] - 0.5*g->dz }, Pp[3] = { Pc[0], Pc[1], Pc[2] + 0.5*g->dz };", 2, 0,
+        "double Pm[3] = { Pc[0], Pc[1], Pc[2] - 0.5*g->dz }, Pp[3] = { Pc[0], Pc[1], Pc[2] + 0.5*g->dz };", 1, 0,
         "double Pm[3] = { Pc[0], Pc[1], Pc[2] - 0.45*g->dz }, Pp[3] = { Pc[0], Pc[1], Pc[2] + 0.45*g->dz };",
         [(T1.test_p4_golden_3d, {})]),
     "arc_row_coordinate_over_a": (
