@@ -77,3 +77,5 @@ int ctsf_launch_fp(const ct_geom *g, const float *d_vol, float *d_proj, int batc
 // transposes d_vol into d_volT ([batch][nz][nx][ny]); returns the number of launches, or -1
 int ctsf_fp_transpose(const ct_geom *g, const float *d_vol, float *d_volT, int batch, void *stream);
 bool ctsf_fp_needs_transpose(const ct_geom *g, int view_begin, int view_stride, int view_count);
+// CTAs the forward kernel launches for `view_count` views of one image (the host pipeline sizes its chunks with it)
+long ctsf_fp_cta_count(const ct_geom *g, int view_count);

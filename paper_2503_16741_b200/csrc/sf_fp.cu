@@ -106,7 +106,7 @@ __device__ __forceinline__ void fp_round_rows(uint32_t ca, float w, const float 
     }
 }
 
-template <int DIM, int ARC, int NB, int UNT, int MODEL>
+template <int DIM, int ARC, int NB, int UNT, int MODEL, int QS = 0>
 __global__ void __launch_bounds__(32 * FPW, FMINB)
 fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ vol,
                const float *__restrict__ volT, float *__restrict__ proj, int view_begin, int view_stride,
@@ -118,8 +118,10 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
     __shared__ SfView sviews[FPW];
     __shared__ Ray srays[FPW][6];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int item = blockIdx.x * FPW + warp;
-    if (item >= n_items) return;                     // warps are independent: no block barrier below
+    // QS (2-D, small problems): the FPW warps of a CTA share ONE item and split its slabs (warp w takes slabs w, w + FPW,
+    // ...); their private tiles are summed in warp order at the end.  Otherwise every warp has an item of its own.
+    const int item = QS ? (int)blockIdx.x : (int)blockIdx.x * FPW + warp;
+    if (item >= n_items) return;                     // warps are independent: no block barrier below (QS: CTA-uniform)
     // item order: groups of FVG consecutive views; within a group tile-major, view fastest -- the
     // warps of one CTA (and the next FVG/FPW - 1 CTAs) sweep the SAME tile of neighbouring views, whose
     // frusta nearly coincide, so the volume is pulled through L1/L2 once per group of views instead of
@@ -176,7 +178,7 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
     const int zstride = np * nq;
     const float v_ap = v.ap, v_bp = v.bp, v_cp = v.cp, v_az = v.az, v_bz = v.bz, v_cz = v.cz;
 
-    for (int iq = 0; iq < nq; ++iq) {
+    for (int iq = QS ? warp : 0; iq < nq; iq += QS ? FPW : 1) {
         // ---- voxel region of this slab that can touch the tile (warp-uniform) --------------------
         // The tile's frustum cuts the slab in a quadrilateral whose rows are skewed (the row coordinate
         // depends on depth, hence on p): the region is swept in sheared coordinates (p, z' = z - shift(p)).
@@ -454,6 +456,18 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
         float *o = proj + (size_t)b0 * proj_bstride + ((size_t)jview * pr.nv + l0) * pr.nu + k0;
         for (int l = 0; l < tlh; ++l)
             for (int k = lane; k < tkw; k += 32) o[(size_t)l * pr.nu + k] = tile[l * FTK + k];
+    } else if (QS) {
+        __syncthreads();                             // all FPW partial tiles of this item are complete
+#pragma unroll
+        for (int bb = 0; bb < NB; ++bb) {
+            float *o = proj + (size_t)(b0 + bb) * proj_bstride + (size_t)jview * pr.nu + k0;
+            for (int k = threadIdx.x; k < tkw; k += 32 * FPW) {
+                float sum = 0.0f;
+#pragma unroll
+                for (int w = 0; w < FPW; ++w) sum += smem[w * (ROWS * FTK) + bb * FTK + k];     // fixed order
+                o[k] = sum;
+            }
+        }
     } else {
 #pragma unroll
         for (int bb = 0; bb < NB; ++bb) {
@@ -481,12 +495,17 @@ void launch_fp(const ct_geom *g, const float *d_vol, const float *d_volT, float 
         : g->model == 1
         ? (hoist ? fp_band_kernel<DIM, ARC, NB, DIM == 3 ? 1 : 0, 1> : fp_band_kernel<DIM, ARC, NB, 0, 1>)
         : (hoist ? fp_band_kernel<DIM, ARC, NB, DIM == 3 ? 1 : 0, 0> : fp_band_kernel<DIM, ARC, NB, 0, 0>);
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const long n_items = (long)tiles_k * bands_l * ((vc + FVG - 1) / FVG) * FVG;
+    // 2-D problems with fewer warp items than the machine holds (148 SMs x 24 warps): split every item's slabs over
+    // the warps of a CTA (config 1: 768 items -> 768 CTAs instead of 96)
+    const bool qsplit = DIM == 2 && n_items * groups < 148L * FPW * FMINB;
+    if (qsplit) kern = g->model == 1 ? fp_band_kernel<DIM, ARC, NB, 0, 1, DIM == 2 ? 1 : 0>
+                                     : fp_band_kernel<DIM, ARC, NB, 0, 0, DIM == 2 ? 1 : 0>;
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     // testing aid: fp_pad = <voxels> widens the swept voxel region; the result must not change beyond
     // summation order (tests/test_gpu_fullsize.py uses it to prove that the tight region misses nothing)
     const float region_pad = g_ctsf_debug.fp_pad;
-    dim3 grid((unsigned)((n_items + FPW - 1) / FPW), groups, 1);
+    dim3 grid((unsigned)(qsplit ? n_items : (n_items + FPW - 1) / FPW), groups, 1);
     kern<<<grid, 32 * FPW, smem, st>>>(pr, g->d_fp, d_vol + (size_t)b0 * vbs,
                                        d_volT ? d_volT + (size_t)b0 * vbs : nullptr,
                                        d_proj + (size_t)b0 * pbs, vb, vs, tiles_k, bands_l, (int)n_items, vc, vbs, pbs, region_pad,
@@ -527,6 +546,13 @@ int launch_fp_batches(const ct_geom *g, const float *d_vol, const float *d_volT,
 }
 
 }  // namespace
+
+long ctsf_fp_cta_count(const ct_geom *g, int view_count)
+{
+    const SfProblem &pr = g->prob;
+    const long tiles = (long)((pr.nu + FTK - 1) / FTK) * (pr.dim == 3 ? (pr.nv + FTL - 1) / FTL : 1);
+    return tiles * ((view_count + FVG - 1) / FVG) * FVG / FPW;
+}
 
 bool ctsf_fp_needs_transpose(const ct_geom *g, int view_begin, int view_stride, int view_count)
 {
