@@ -171,7 +171,7 @@ def main():
     ap.add_argument("--impl", default="ctsf")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--algo", default="SF", choices=["SF", "DD"],
+    ap.add_argument("--algo", default="SF", choices=["SF", "DD", "SF-TT"],
                     help="voxel model: SF (separable footprint, the headline) or DD (distance-driven, row f4)")
     ap.add_argument("--fbp", action="store_true",
                     help="also time recon mode (row f2): ct_fbp_filter + ct_bp_sf_recon on the step's projections")

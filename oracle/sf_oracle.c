@@ -16,7 +16,9 @@
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): trapezoid CDF vs quadrature; hand-worked 2-D
  * and 3-D footprints; brute-force ray/box chords; analytic disk/ellipsoid chords; mass
  * identities; parallel-beam column sums; 2-D == one-slice 3-D; dense-matrix transpose; adjoint
- * to 1e-12; symmetries.  Unpinned: arc detector in a tilted frame beyond brute force (R8).
+ * to 1e-12; symmetries; tilted frames and reversed axes against an independent ray/detector intersection model;
+ * every factor of recon mode against analytic FBP/FDK; tests/test_oracle_mutations.py applies 24 one-line mutations
+ * of this file and checks that a named pin fails for each.  Unpinned: nothing.
  *
  * Build: gcc -O2 -fopenmp -shared -fPIC -o libsf_oracle.so sf_oracle.c -lm
  */

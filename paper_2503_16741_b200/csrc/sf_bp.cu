@@ -439,8 +439,8 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
 //      row loops run over max(K_a, K_b) x max(L_a, L_b); each footprint is cut at its own last cell edges, so the
 //      cells past them weigh exactly 0 (their loads stay inside the CTA's shared memory);
 //  (2) the views flow through a ring of BP2_STAGES tile buffers guarded by mbarrier pairs: full[s] completes when
-//      the TMA bytes of the view have landed (warp 0 stages the view's parameters and the brick's shadow and arms
-//      it), empty[s] when all warps have finished reading the stage.  No __syncthreads in the view loop: warps
+//      the TMA bytes of the view have landed (one warp, in rotation, stages the view's parameters and the brick's
+//      shadow and arms it), empty[s] when all warps have finished reading the stage.  No __syncthreads in the view loop: warps
 //      drift up to a view apart instead of waiting for the slowest one at every view (0.9 barrier stalls per
 //      issued instruction in the round-1 kernel).  Shadows larger than one box (rare) fall back to block-wide
 //      cp.async staging inside the view, which re-synchronises the CTA.
@@ -533,7 +533,9 @@ bp_brick2_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__
     int s = 0, sp = BP2_STAGES - 1;           // slot of view j / of view j + BP2_STAGES - 1
     uint32_t par = 0u;                        // phase parity of slot s's current use
     for (int j = j_lo; j < j_hi; ++j) {
-        if (warp == 0 && j + BP2_STAGES - 1 < j_hi) {
+        // the producer role rotates over the warps (view j + 2 is staged by warp (j mod 8)), so that no warp is
+        // systematically behind the others by the staging work
+        if (warp == ((j - j_lo) & (BRICK_THREADS / 32 - 1)) && j + BP2_STAGES - 1 < j_hi) {
             // slot sp held view j - 1: every warp must have left it (its first use needs no wait)
             if (j > j_lo) mbar_wait(&empty[sp], (uint32_t)(((j - 1 - j_lo) / BP2_STAGES) & 1));
             produce(j + BP2_STAGES - 1, sp);
@@ -687,7 +689,7 @@ int launch_brick(const ct_geom *g, const float *d_proj, float *d_vol, int batch,
                        (g->fp_hoist_ok || (g->all_untilted && g_ctsf_debug.bp_forcehoist)) && g->model != 2;
     // general frames: the packed two-voxel kernel (needs the TMA path); the testing aid bp_scalar keeps the
     // one-voxel-per-thread kernel
-    const bool packed = !hoist && use_tma == 3 && !g_ctsf_debug.bp_scalar && g->model != 2;
+    const bool packed = !hoist && use_tma == 3 && !g_ctsf_debug.bp_scalar && g->model == 0;   // DD: its rectangle footprint has no packed form worth having (measured 306 vs 289 ms)
     auto kern = g->model == 2 ? (recon ? bp_brick_kernel<ARC, 1, 0, 2> : bp_brick_kernel<ARC, 0, 0, 2>)
         : g->model == 1
         ? (hoist ? (recon ? bp_brick_kernel<ARC, 1, 1, 1> : bp_brick_kernel<ARC, 0, 1, 1>)
