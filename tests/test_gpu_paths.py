@@ -440,3 +440,65 @@ def test_view_sharded_operators_world_size_1():
     assert (xb - full).abs().max().item() <= 3e-6 * full.abs().max().item()
     assert torch.equal(geom.bp_sharded(y, 0, 1), full)
     geom.close()
+
+
+def test_bench_view_sharded_mode_single_rank():
+    """bench.py --shard views at N = 1: runs, prints one contract line, strong scaling label."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--shard", "views", "--config", "1", "--steps", "2",
+                          "--warmup", "3", "--no-cpu"], capture_output=True, text=True, timeout=600, cwd=root)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["scaling"] == "strong" and d["value"] > 0 and d["gpu_launches"] > 0
+    assert d["shard"]["mode"] == "views" and len(d["shard"]["per_rank_ms_fp_bp_allreduce"]) == 1
+    assert d["roofline"]["peak"] > 50.0 and "measured" in d["roofline"]["peak_src"]
+
+
+_TWO_GPU_WORKER = r'''
+import os, sys
+sys.path.insert(0, sys.argv[1])
+import numpy as np, torch, torch.distributed as dist
+from paper_2503_16741_b200 import workloads as W
+from paper_2503_16741_b200.projector import Geometry
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+torch.cuda.set_device(int(os.environ["LOCAL_RANK"]))
+dist.init_process_group("nccl", device_id=torch.device("cuda", int(os.environ["LOCAL_RANK"])))
+c = W.make_config(4, nx=40, ny=36, nz=32, nu=96, nv=88, n_views=13)
+geom = Geometry(W.geom_keys(c))
+x = torch.from_numpy(W.make_phantom(c)).cuda()
+y_full = geom.fp(x)                                   # every rank: the unsharded reference
+(vb, vs, vc), y_mine = geom.fp_sharded(x, rank, world)
+assert torch.equal(y_mine, y_full[:, vb:vb + vc])
+xb = geom.bp_sharded(y_mine, rank, world)             # ct_bp_sf_views + one NCCL all-reduce
+full = geom.bp(y_full)
+assert (xb - full).abs().max().item() <= 3e-6 * full.abs().max().item()
+dist.destroy_process_group()
+print("ok")
+'''
+
+
+def test_view_sharded_operators_two_gpus(tmp_path):
+    """The same identities over NCCL when the box has two GPUs (skipped on the single-GPU boxes of this run)."""
+    import os
+    import socket
+    import subprocess
+    import sys
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "worker.py"
+    script.write_text(_TWO_GPU_WORKER)
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    out = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                          "--master-addr", "127.0.0.1", "--master-port", str(port), str(script), root],
+                         capture_output=True, text=True, timeout=900)
+    assert out.returncode == 0 and out.stdout.count("ok") == 2, (out.stdout[-1000:], out.stderr[-2000:])

@@ -1,9 +1,12 @@
 """Pins for the oracle's "recon" mode (readings R23, R24): filtered
 backprojection x = (pi/N) B(filter(p)) of ANALYTIC projections (closed-form chord lengths, cell-centre rays --
 nothing computed by a projector) must return the attenuation value inside a uniform object.  Fan-beam FBP and
-the mid-plane of circular cone-beam FDK are exact inversions, so the only error is discretisation; a dropped
-cosine weight, a wrong filter scale, a missing (pi/N) or a wrong depth weight each shift the plateau by >= 3 %.
-CPU only (-m "not gpu")."""
+circular cone-beam FDK of a z-invariant object are exact inversions, so the only error is discretisation.
+The first group of tests (objects near the axis, mid-plane) pins the overall scale: filter normalisation, (pi/N),
+d R / a^2.  It does NOT see the cosine pre-weights, the equi-angular taps or the (a^2 + b^2) depth weight, which are
+within 0.1 % of 1 there (round 1 claimed otherwise; one-line mutations of each survived).  The second group, at the
+end of the file, isolates each of those factors: dropping one moves the plateau by 1.5-3.9 % against tolerances of
+0.3-0.5 % (tests/test_oracle_mutations.py proves it on mutated builds).  CPU only (-m "not gpu")."""
 import math
 
 import numpy as np
