@@ -128,6 +128,8 @@ CTSF_API int ctsf_debug_set(const char *name, double value)
     else if (n == "bp_tma") d.bp_tma = (int)value;
     else if (n == "bp_chunk") d.bp_chunk = (int)value;
     else if (n == "bp_scalar") d.bp_scalar = (int)value;
+    else if (n == "host_fp_chunks") d.host_fp_chunks = (int)value;
+    else if (n == "host_bp_chunks") d.host_bp_chunks = (int)value;
     else return -1;
     return 0;
 }
@@ -317,14 +319,18 @@ static ct_status_t host_op(const ct_geom_t *g, const float *h_in, float *h_out, 
     ct_status_t rc = CT_OK;
     int launches = 0;
     constexpr int MAX_CHUNKS = 8;
-    int n_chunks = (pr.dim == 3 && batch == 1) ? (pr.n_views >= 64 ? MAX_CHUNKS : (pr.n_views >= 8 ? 2 : 1)) : 1;
+    int n_chunks = (pr.dim == 3 && batch == 1) ? (pr.n_views >= 64 ? 6 : (pr.n_views >= 8 ? 2 : 1)) : 1;
     if (fwd && n_chunks > 1) {
         // A forward chunk must still fill the machine for several waves: the work per detector tile is very uneven
         // (edge tiles see little of the volume), and a one-wave launch runs at the pace of its slowest CTA (measured
-        // at config 2: 45 of 360 views take 17.5 ms, all 360 take 72.8 ms).  >= 6 waves of 148 x 3 CTAs per chunk.
-        const long per_chunk = 6L * 148 * 3;
+        // at config 2: 45 of 360 views take 17.5 ms, all 360 take 72.8 ms; config 4: 8 chunks 733 ms, 3 chunks 694 ms for A).  >= 18 waves of 148 x 3 CTAs per chunk.
+        const long per_chunk = 18L * 148 * 3;
         const long fit = ctsf_fp_cta_count(g, pr.n_views) / per_chunk;
         n_chunks = (int)(fit < 1 ? 1 : (fit > MAX_CHUNKS ? MAX_CHUNKS : fit));
+    }
+    {   // testing aids: force the number of view chunks of the 3-D batch-1 pipeline
+        const int forced = fwd ? g_ctsf_debug.host_fp_chunks : g_ctsf_debug.host_bp_chunks;
+        if (forced > 0 && pr.dim == 3 && batch == 1) n_chunks = forced > MAX_CHUNKS ? MAX_CHUNKS : (forced > pr.n_views ? pr.n_views : forced);
     }
     auto ok = [&](cudaError_t e) { if (e != cudaSuccess && rc == CT_OK) rc = CT_ERR_CUDA; return e == cudaSuccess; };
     if (n_chunks == 1) {

@@ -98,14 +98,17 @@ def test_thin_volumes_and_detectors():
 
 def test_host_buffer_entry_points():
     """ct_fp_sf_host / ct_bp_sf_host (the e2e path of bench.py): view-chunked copy/compute pipeline for
-    3-D batch 1 (8 chunks at >= 64 views, A^T accumulating chunk by chunk), plain path otherwise; results
+    3-D batch 1 (A^T: 6 chunks at >= 64 views, accumulating chunk by chunk; A: chunks of >= 18 waves of CTAs, i.e.
+    one chunk at test sizes -- 5 chunks are forced here to exercise the pipeline), plain path otherwise; results
     must equal the device-pointer operators bit for bit (A) / to rounding of the chunked sum (A^T) and
     match the oracle within the usual tolerances."""
     from paper_2503_16741_b200 import binding as B
     from paper_2503_16741_b200.projector import Geometry
-    for index, shrink in ((4, dict(nx=36, ny=40, nz=30, nu=100, nv=90, n_views=67)),
-                          (2, dict(nx=30, ny=30, nz=20, nu=64, nv=60, n_views=9)),
-                          (5, dict(nx=64, ny=60, nu=150, n_views=20, batch=3))):
+    for index, shrink, fp_chunks in ((4, dict(nx=36, ny=40, nz=30, nu=100, nv=90, n_views=67), 5),
+                                     (4, dict(nx=36, ny=40, nz=30, nu=100, nv=90, n_views=67), 0),
+                                     (2, dict(nx=30, ny=30, nz=20, nu=64, nv=60, n_views=9), 0),
+                                     (5, dict(nx=64, ny=60, nu=150, n_views=20, batch=3), 0)):
+        B.debug_set("host_fp_chunks", fp_chunks)
         c = W.make_config(index, **shrink)
         g = W.geom_keys(c)
         x = W.make_phantom(c)
@@ -294,6 +297,7 @@ def test_host_buffer_entry_points_odd_sizes():
     from paper_2503_16741_b200.projector import Geometry
     for index, shrink in ((2, dict(nx=26, ny=24, nz=18, nu=150, nv=101, n_views=11)),
                           (4, dict(nx=30, ny=28, nz=26, nu=101, nv=91, n_views=67))):
+        B.debug_set("host_fp_chunks", 7 if index == 4 else 2)      # chunk offsets v0 * nv * nu: odd multiples of 4 bytes
         c = W.make_config(index, **shrink)
         g = W.geom_keys(c)
         x = W.make_phantom(c)
