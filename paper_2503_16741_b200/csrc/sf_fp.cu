@@ -106,6 +106,15 @@ __device__ __forceinline__ void fp_round_rows(uint32_t ca, float w, const float 
     }
 }
 
+// the same for footprints of at most three rows (untilted frames with cells larger than half a voxel's shadow:
+// configs 2, 3): three unconditional rows instead of four
+__device__ __forceinline__ void fp_round_rows3(uint32_t ca, float w, const float *f2)
+{
+    constexpr int RB = FTK * 4;
+    const float c0 = lds_f32(ca), c1 = lds_f32(ca + RB), c2 = lds_f32(ca + 2 * RB);
+    sts_f32(ca, fmaf(w, f2[0], c0)); sts_f32(ca + RB, fmaf(w, f2[1], c1)); sts_f32(ca + 2 * RB, fmaf(w, f2[2], c2));
+}
+
 template <int DIM, int ARC, int NB, int UNT, int MODEL, int QS = 0>
 __global__ void __launch_bounds__(32 * FPW, FMINB)
 fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ vol,
@@ -293,7 +302,14 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
                         const int Kall = __reduce_max_sync(FULL, live ? j_b + 1 : 0);
                         for (int ser = 0; ser < n_serial; ++ser) {
                             const bool mine = live && (ok || lane == ser);
-                            if (Lmax <= FLM) {
+                            if (Lmax <= 3) {
+#pragma unroll
+                                for (int jk = 0; jk < FKR; ++jk) {
+                                    if (jk >= Kall) break;               // warp-uniform
+                                    if (mine && jk >= j_a && jk <= j_b) fp_round_rows3(ca + 4u * jk, f1[jk] * ax, f2);
+                                    __syncwarp();
+                                }
+                            } else if (Lmax <= FLM) {
 #pragma unroll
                                 for (int jk = 0; jk < FKR; ++jk) {
                                     if (jk >= Kall) break;               // warp-uniform
