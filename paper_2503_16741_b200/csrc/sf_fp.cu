@@ -70,7 +70,10 @@ __device__ __forceinline__ Ray tile_ray(const SfView &v, float kf, float lf)
 // p are interleaved half a region apart; the kernel verifies both per pass with a warp match and
 // serialises the pass otherwise), so within a round no two lanes touch the same cell; rounds are
 // separated by __syncwarp().  Summation order is fixed => deterministic.
-constexpr int FPW = 8;            // warps per CTA
+constexpr int FPW = 8;            // warps per CTA (slab-split 2-D kernels; unit of the item groups)
+#ifndef FP_WPC
+#define FP_WPC 8                     // warps per CTA of the general kernels (measured: 1 warp per CTA is 1.5-5 % slower)
+#endif
 constexpr int FVG = 48;           // views per item group (multiple of FPW): consecutive CTAs sweep one tile of FVG views
 constexpr int FMINB = 3;          // CTAs per SM the register budget is sized for
 constexpr int FTK = 64;           // cells per warp tile
@@ -116,7 +119,7 @@ __device__ __forceinline__ void fp_round_rows3(uint32_t ca, float w, const float
 }
 
 template <int DIM, int ARC, int NB, int UNT, int MODEL, int QS = 0>
-__global__ void __launch_bounds__(32 * FPW, FMINB)
+__global__ void __launch_bounds__(32 * (QS ? FPW : FP_WPC), FMINB * FPW / (QS ? FPW : FP_WPC))
 fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ vol,
                const float *__restrict__ volT, float *__restrict__ proj, int view_begin, int view_stride,
                int tiles_k, int bands_l, int n_items, int n_views_sel, size_t vol_bstride, size_t proj_bstride,
@@ -124,12 +127,17 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
 {
     constexpr int ROWS = DIM == 3 ? FTL + FLM : NB;
     extern __shared__ float smem[];
-    __shared__ SfView sviews[FPW];
-    __shared__ Ray srays[FPW][6];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // Warps per CTA.  Every warp is independent (own tile, own view parameters).  With one warp per CTA `warp` is the
+    // constant 0 and every per-warp shared-memory address a compile-time offset (with 8 warps ptxas, at its 80-register
+    // budget, keeps re-deriving them from threadIdx: 5-7 % of the executed instructions) -- yet measured on B200 the
+    // 1-warp CTAs were slower (config 4: 673.6 vs 664.2 ms; configs 2, 3, 5: +4 %, +5.5 %, +5 %), so FP_WPC stays 8.
+    constexpr int WPC = QS ? FPW : FP_WPC;
+    __shared__ SfView sviews[WPC];
+    __shared__ Ray srays[WPC][6];
+    const int lane = threadIdx.x & 31, warp = WPC == 1 ? 0 : (int)(threadIdx.x >> 5);
     // QS (2-D, small problems): the FPW warps of a CTA share ONE item and split its slabs (warp w takes slabs w, w + FPW,
     // ...); their private tiles are summed in warp order at the end.  Otherwise every warp has an item of its own.
-    const int item = QS ? (int)blockIdx.x : (int)blockIdx.x * FPW + warp;
+    const int item = QS ? (int)blockIdx.x : (int)blockIdx.x * WPC + warp;
     if (item >= n_items) return;                     // warps are independent: no block barrier below (QS: CTA-uniform)
     // item order: groups of FVG consecutive views; within a group tile-major, view fastest -- the
     // warps of one CTA (and the next FVG/FPW - 1 CTAs) sweep the SAME tile of neighbouring views, whose
@@ -501,7 +509,8 @@ void launch_fp(const ct_geom *g, const float *d_vol, const float *d_volT, float 
     const int tiles_k = (pr.nu + FTK - 1) / FTK, bands_l = DIM == 3 ? (pr.nv + FTL - 1) / FTL : 1;
     const size_t vbs = (size_t)pr.nx * pr.ny * pr.nz, pbs = (size_t)vc * pr.nv * pr.nu;
     constexpr int ROWS = DIM == 3 ? FTL + FLM : NB;
-    const size_t smem = (size_t)FPW * ROWS * FTK * sizeof(float);
+    const int wpc_general = FP_WPC;
+    size_t smem = (size_t)wpc_general * ROWS * FTK * sizeof(float);
     // testing aids (CtsfDebug): fp_nohoist never uses the untilted fast path; fp_forcehoist uses it for every
     // untilted 3-D geometry, also when footprints exceed its register windows (exercises its overflow branch)
     const bool hoist = DIM == 3 && !g_ctsf_debug.fp_nohoist &&
@@ -517,12 +526,14 @@ void launch_fp(const ct_geom *g, const float *d_vol, const float *d_volT, float 
     const bool qsplit = DIM == 2 && n_items * groups < 148L * FPW * FMINB;
     if (qsplit) kern = g->model == 1 ? fp_band_kernel<DIM, ARC, NB, 0, 1, DIM == 2 ? 1 : 0>
                                      : fp_band_kernel<DIM, ARC, NB, 0, 0, DIM == 2 ? 1 : 0>;
+    const int wpc = qsplit ? FPW : wpc_general;
+    smem = (size_t)wpc * ROWS * FTK * sizeof(float);
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     // testing aid: fp_pad = <voxels> widens the swept voxel region; the result must not change beyond
     // summation order (tests/test_gpu_fullsize.py uses it to prove that the tight region misses nothing)
     const float region_pad = g_ctsf_debug.fp_pad;
-    dim3 grid((unsigned)(qsplit ? n_items : (n_items + FPW - 1) / FPW), groups, 1);
-    kern<<<grid, 32 * FPW, smem, st>>>(pr, g->d_fp, d_vol + (size_t)b0 * vbs,
+    dim3 grid((unsigned)(qsplit ? n_items : (n_items + wpc - 1) / wpc), groups, 1);
+    kern<<<grid, 32 * wpc, smem, st>>>(pr, g->d_fp, d_vol + (size_t)b0 * vbs,
                                        d_volT ? d_volT + (size_t)b0 * vbs : nullptr,
                                        d_proj + (size_t)b0 * pbs, vb, vs, tiles_k, bands_l, (int)n_items, vc, vbs, pbs, region_pad,
                                        g_ctsf_debug.fp_serial ? 1 : 0);   // testing aid: take the lane-serial branch
