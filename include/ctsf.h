@@ -16,7 +16,10 @@
  *  - outputs are OVERWRITTEN (y = A x, x = A^T y), never accumulated into;
  *  - device entry points are asynchronous on `stream`: no host synchronisation, no host<->device
  *    copy of image data; scratch memory, when needed, comes from the stream-ordered allocator;
- *  - every function returns a ct_status_t; nothing throws across the boundary.
+ *  - every function returns a ct_status_t; nothing throws across the boundary;
+ *  - inputs are expected to be finite: the kernels multiply cells just outside a footprint by a weight that is
+ *    exactly 0 instead of skipping them, so a NaN / Inf in the input may reach outputs up to one footprint width
+ *    beyond the cells and voxels it mathematically touches (finite inputs: results as documented, deterministic).
  */
 #ifndef CTSF_H
 #define CTSF_H
