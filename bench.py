@@ -224,6 +224,7 @@ def main():
     peak_flops = [B.ct_measure_fp32_peak(k, stream.cuda_stream)[0] for k in (0, 1, 0, 1)]
     peak_clocks = peak_sampler.stop() if peak_sampler else None
     peak_scalar, peak_packed = max(peak_flops[0::2]) / 1e12, max(peak_flops[1::2]) / 1e12
+    mix_ffma2_ffma, mix_ffma2_fmnmx = [B.ct_measure_fp32_peak(k, stream.cuda_stream)[0] / 1e12 for k in (2, 3)]
 
     def step():
         geom.fp(x, views=sel, out=y)
@@ -367,6 +368,7 @@ def main():
                                                               peak_clocks.get("sm_mhz") if peak_clocks else "?",
                                                               pk["sm_max_mhz"], pk["fp32_tflops_nominal"]),
                          "peak_scalar_ffma": peak_scalar, "peak_packed_ffma2": peak_packed,
+                         "mix_ffma2_with_ffma_tflops": mix_ffma2_ffma, "mix_ffma2_with_fmnmx_tflops": mix_ffma2_fmnmx,
                          "flop_per_update": FLOP_PER_UPDATE[args.config],
                          "flop_per_update_src": "algorithmic count of S1-S5 per nominal update (DESIGN.md section 7)",
                          "executed_flop_per_update": mdom.get("flop_per_update"),

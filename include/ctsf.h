@@ -156,7 +156,8 @@ CTSF_API int32_t ct_last_launch_count(const ct_geom_t *geom);
  * roofline that binds this path (it is bound by fp32 arithmetic / instruction issue, not by HBM; DESIGN.md
  * "Roofline").  Runs an FMA-only kernel (independent register chains, no memory traffic, 4 waves
  * of one 1024-thread CTA per SM), best of 3, timed with CUDA events on `stream`; SYNCHRONISES `stream`.
- * kind 0: scalar FFMA; kind 1: packed FFMA2 (two FMAs per lane and instruction, sm_100).
+ * kind 0: scalar FFMA; kind 1: packed FFMA2 (two FMAs per lane and instruction, sm_100); kinds 2, 3 (design record, not
+ * peaks): FFMA2 interleaved 1:1 with scalar FFMA / with an ALU-pipe FMNMX -- FMA flops of the mix.
  * *flops_per_s HOST, written; *seconds HOST, optional (duration of the timed launch).
  * Errors: CT_ERR_INVALID_ARG, CT_ERR_ALLOC, CT_ERR_CUDA. */
 CTSF_API ct_status_t ct_measure_fp32_peak(int32_t kind, double *flops_per_s, double *seconds, ct_stream_t stream);
