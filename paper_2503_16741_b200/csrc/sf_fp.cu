@@ -170,7 +170,13 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
         const float kA = (float)k0, kB = (float)(k0 + tkw), lA = (float)l0, lB = (float)(l0 + tlh);
         const float kk = (lane % 3 == 0) ? kA : (lane % 3 == 1 ? kB : 0.5f * (kA + kB));
         const Ray ry = tile_ray<ARC>(v, kk, lane < 3 ? lA : lB);
-        srays[warp][lane] = ry;
+        // stored per unit of q: (dp/dq, sign of dq, dz/dq); sign 0 marks a ray (almost) parallel to the slabs, for which
+        // the whole slab is swept.  The slab loop then needs two FMAs and one compare per ray instead of a reciprocal.
+        const bool flat_ray = fabsf(ry.dq) < 1e-3f * (fabsf(ry.dp) + fabsf(ry.dz));
+        const float inv_dq = flat_ray ? 0.0f : rcp_nr(ry.dq);
+        Ray rn;
+        rn.dp = ry.dp * inv_dq; rn.dq = flat_ray ? 0.0f : (ry.dq > 0.0f ? 1.0f : -1.0f); rn.dz = ry.dz * inv_dq;
+        srays[warp][lane] = rn;
         // direction of the line {k = const, z = const} in the slab plane: the ray minus its z part along v
         float dp = ry.dp, dq = ry.dq;
         if (DIM == 3 && fabsf(v.Vz) > 1e-6f) {
@@ -206,10 +212,9 @@ fp_band_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__re
 #pragma unroll
         for (int r = 0; r < 6; ++r) {
             if (DIM == 2 && r >= 3) break;
-            const Ray ry = srays[warp][r];
-            if (!(ry.dq * dqc > 0.0f) || fabsf(ry.dq) < 1e-3f * (fabsf(ry.dp) + fabsf(ry.dz))) whole = true;
-            const float lam = dqc * rcp_nr(ry.dq);
-            pr_[r] = fmaf(lam, ry.dp, v.Sp); zr_[r] = fmaf(lam, ry.dz, v.Sz);
+            const Ray ry = srays[warp][r];                      // (dp/dq, sign(dq) or 0, dz/dq)
+            if (!(ry.dq * dqc > 0.0f)) whole = true;            // slab behind the source along this ray, or a flat ray
+            pr_[r] = fmaf(dqc, ry.dp, v.Sp); zr_[r] = fmaf(dqc, ry.dz, v.Sz);
             pmin = fminf(pmin, pr_[r]); pmax = fmaxf(pmax, pr_[r]);
         }
         int p_lo = 0, p_hi = np - 1, zs_lo = 0, zs_hi = nz - 1;
