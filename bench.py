@@ -374,6 +374,7 @@ def main():
                          "executed_flop_per_update": mdom.get("flop_per_update"),
                          "executed_frac": (mdom["flop_per_update"] * updates / (dom_ms * 1e-3) / 1e12 / peak)
                                           if mdom.get("flop_per_update") else None,
+                         "issue_slots_busy_pct": mdom.get("issue_active_pct"),
                          "measured_counts_src": mdom.get("src"),
                          "hbm": {"algorithmic_bytes": alg_bytes, "achieved_gbs": alg_bytes / (dom_ms * 1e-3) / 1e9,
                                  "peak_gbs": pk["hbm_gbs"], "frac": alg_bytes / (dom_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
