@@ -702,11 +702,13 @@ int launch_brick(const ct_geom *g, const float *d_proj, float *d_vol, int batch,
     if (packed) cudaFuncSetAttribute(kern2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
     const int nbz = (pr.nz + BZ - 1) / BZ;
     int launches = 0;
-    // The view loop is cut into chunks of ~96 MB of projections, one launch each (every launch after the
-    // first adds to the volume): all bricks sweep one chunk while it sits in the 126 MB L2, instead of
-    // each wave of CTAs streaming the whole projection set from HBM again.
+    // The view loop is cut into chunks of ~288 MB of projections, one launch each (every launch after the first adds
+    // to the volume): all bricks sweep one chunk while most of it stays in the 126 MB L2, instead of each wave of CTAs
+    // streaming the whole projection set from HBM again.  Measured at config 4 (B200, per A^T; time / DRAM read + written):
+    // 40 views per launch 394.8 ms / 13.4 + 8.7 GB; 80: 390.0 / 13.9 + 4.4; 120: 389.1 / 15.0 + 2.9; 240: 389.1 / 22.5 + 1.5;
+    // all 720 in one launch 390.5 / 105 + 0.5.  120 views (283 MB) is the fastest and moves the fewest bytes.
     const size_t view_bytes = (size_t)pr.nu * pr.nv * sizeof(float) * batch;
-    int chunk = (int)((96u << 20) / (view_bytes ? view_bytes : 1));
+    int chunk = (int)((288u << 20) / (view_bytes ? view_bytes : 1));
     if (chunk < 8) chunk = 8;
     if (g_ctsf_debug.bp_chunk > 0) chunk = g_ctsf_debug.bp_chunk;
     for (int j_lo = 0; j_lo < vc || (vc == 0 && j_lo == 0); j_lo += chunk) {
