@@ -171,7 +171,7 @@ def debug_set(name, value=1):
 
 def ct_measure_fp32_peak(kind=0, stream=0):
     """Measured fp32 FMA throughput of the current device: (flop/s, seconds of the timed launch).
-    kind 0: scalar FFMA, 1: packed FFMA2."""
+    kind 0: scalar FFMA, 1: packed FFMA2; 2, 3 (design record): FFMA2 interleaved with scalar FFMA / with FMNMX."""
     f, t = ctypes.c_double(0.0), ctypes.c_double(0.0)
     _check(lib().ct_measure_fp32_peak(int(kind), ctypes.byref(f), ctypes.byref(t), stream), "ct_measure_fp32_peak")
     return f.value, t.value

@@ -506,3 +506,16 @@ def test_view_sharded_operators_two_gpus(tmp_path):
                           "--master-addr", "127.0.0.1", "--master-port", str(port), str(script), root],
                          capture_output=True, text=True, timeout=900)
     assert out.returncode == 0 and out.stdout.count("ok") == 2, (out.stdout[-1000:], out.stderr[-2000:])
+
+
+def test_fp32_peak_microbenchmark():
+    """ct_measure_fp32_peak (the roofline's measured denominator): plausible on any Blackwell-class part, packed >=
+    scalar, the FFMA2 / FFMA mix below both, bad arguments rejected."""
+    f0, t0 = B.ct_measure_fp32_peak(0)
+    f1, _ = B.ct_measure_fp32_peak(1)
+    f2, _ = B.ct_measure_fp32_peak(2)
+    f3, _ = B.ct_measure_fp32_peak(3)
+    assert 20e12 < f0 < 120e12 and 0.9 * f0 < f1 < 120e12 and t0 > 0
+    assert f2 < 0.95 * f1 and f3 < 0.95 * f1
+    with pytest.raises(B.CtError):
+        B.ct_measure_fp32_peak(4)
