@@ -45,7 +45,8 @@ typedef enum {
     CT_ERR_GEOMETRY = 2,      /* axes not unit/orthogonal, detector behind the source, arc detector not
                                  centred on the source axis, volume reaching the source plane, a 2-D
                                  geometry with out-of-plane components */
-    CT_ERR_UNSUPPORTED = 3,   /* problem too large for 32-bit indexing of one image */
+    CT_ERR_UNSUPPORTED = 3,   /* problem too large for 32-bit indexing of one image, or for the fixed scratch of
+                                 ct_fp_sf_noalloc */
     CT_ERR_ALLOC = 4,         /* host or device allocation failed */
     CT_ERR_CUDA = 5           /* a CUDA runtime call or kernel launch failed (no usable device, ...) */
 } ct_status_t;
@@ -96,6 +97,29 @@ CTSF_API ct_status_t ct_geom_destroy(ct_geom_t *geom);
  * along x read is owned by the geometry, grown on first use and kept until ct_geom_destroy). */
 CTSF_API ct_status_t ct_fp_sf(const ct_geom_t *geom, const float *d_vol, float *d_proj,
                      int32_t batch, ct_stream_t stream);
+
+/* y = A x like ct_fp_sf -- same arguments, layouts, kernels and results -- for callers that are not allowed to
+ * allocate device memory once they are running: a reconstruction loop inside a process whose GPU memory is already
+ * owned by another allocator (a framework's caching pool, a fixed budget on a shared GPU), a loop with a latency
+ * bound that cannot afford the device-wide stall of a cudaMalloc, a service whose policy forbids growth after
+ * start-up.  Create the geometry at start-up (ct_geom_create does allocate); this call never does: no cudaMalloc,
+ * cudaFree, stream-ordered allocation or allocating library routine, on the first call or any later one.
+ * Its only scratch, the xy-transposed copy of the volume that views along x read, lives in a fixed array inside the
+ * library image: 16 MiB of every GPU that uses libctsf, held until the process exits.  What follows from that:
+ *  - limit: batch * nz * ny * nx <= CT_FP_SF_NOALLOC_MAX_VOXELS (e.g. one 160^3 volume, sixteen 512^2 images);
+ *    anything larger is refused with CT_ERR_UNSUPPORTED before any work is queued -- use ct_fp_sf for it;
+ *  - the GPU the geometry was created on must be the current device (else CT_ERR_INVALID_ARG);
+ *  - the first call on each GPU looks up the array's device address (cudaGetSymbolAddress, which may load the
+ *    library's device code): make that first call before starting any stream capture.  Later calls do no set-up;
+ *  - every call on a GPU, whatever its geometry or stream, uses the same array.  Calls queued on ONE stream are safe
+ *    (each call rewrites the part of the array it reads; nothing needs clearing, stale contents are never read).
+ *    Calls that may overlap on the GPU -- different streams, different host threads -- race on it and corrupt each
+ *    other's results: order them yourself (one stream, or events), or use ct_fp_sf there.
+ * d_vol: DEVICE, read; d_proj: DEVICE, written (every element exactly once); both caller-owned.  Asynchronous on
+ * `stream`.  Errors: CT_ERR_INVALID_ARG, CT_ERR_UNSUPPORTED (over the limit), CT_ERR_CUDA. */
+#define CT_FP_SF_NOALLOC_MAX_VOXELS 4194304
+CTSF_API ct_status_t ct_fp_sf_noalloc(const ct_geom_t *geom, const float *d_vol, float *d_proj,
+                             int32_t batch, ct_stream_t stream);
 
 /* x = A^T y (Eq. 2): the exact transpose of the weights of ct_fp_sf.
  * d_proj: DEVICE, read; d_vol: DEVICE, written (every element exactly once).  Asynchronous. */

@@ -17,7 +17,9 @@ STATUS_NAMES = {0: "CT_OK", 1: "CT_ERR_INVALID_ARG", 2: "CT_ERR_GEOMETRY", 3: "C
                 4: "CT_ERR_ALLOC", 5: "CT_ERR_CUDA"}
 EXPORTS = ("ct_geom_create", "ct_geom_destroy", "ct_fp_sf", "ct_bp_sf", "ct_fp_sf_views", "ct_bp_sf_views",
            "ct_fp_sf_host", "ct_bp_sf_host", "ct_fbp_filter", "ct_fbp_filter_views", "ct_bp_sf_recon",
-           "ct_bp_sf_recon_views", "ct_fbp_sf", "ct_measure_fp32_peak", "ct_last_launch_count", "ct_status_string")
+           "ct_bp_sf_recon_views", "ct_fbp_sf", "ct_measure_fp32_peak", "ct_last_launch_count", "ct_status_string",
+           "ct_fp_sf_noalloc")
+CT_FP_SF_NOALLOC_MAX_VOXELS = 4194304          # include/ctsf.h
 
 
 class CtError(RuntimeError):
@@ -71,6 +73,8 @@ def lib():
         L.ct_status_string.restype = ctypes.c_char_p
         for name in EXPORTS[:14]:
             getattr(L, name).restype = ctypes.c_int
+        L.ct_fp_sf_noalloc.argtypes = [P, P, P, I, P]
+        L.ct_fp_sf_noalloc.restype = ctypes.c_int
         _lib = L
     return _lib
 
@@ -119,6 +123,18 @@ def ct_fp_sf(handle, d_vol, d_proj, batch, stream=0):
 
 def ct_bp_sf(handle, d_proj, d_vol, batch, stream=0):
     _check(lib().ct_bp_sf(handle, d_proj, d_vol, int(batch), stream), "ct_bp_sf")
+
+
+def ct_fp_sf_noalloc(handle, d_vol, d_proj, batch, stream=0):
+    """ct_fp_sf for callers that may not allocate device memory while running (GPU memory owned by another pool, a
+    latency-bound loop, a no-growth policy): same arguments and results, scratch in a fixed 16 MiB array of the library
+    instead of a cudaMalloc.  Refuses batch * nz * ny * nx > CT_FP_SF_NOALLOC_MAX_VOXELS; all calls on a GPU share the
+    array, so keep them on one stream (overlapping calls race).  Make the first call on a GPU outside stream capture."""
+    status = lib().ct_fp_sf_noalloc(handle, d_vol, d_proj, int(batch), stream)
+    if status == 3:
+        raise CtError(status, "ct_fp_sf_noalloc (batch * nz * ny * nx exceeds the fixed scratch of %d voxels; "
+                              "use ct_fp_sf)" % CT_FP_SF_NOALLOC_MAX_VOXELS)
+    _check(status, "ct_fp_sf_noalloc")
 
 
 def ct_fp_sf_views(handle, d_vol, d_proj, batch, view_begin, view_stride, view_count, stream=0):

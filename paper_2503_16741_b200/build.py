@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libctsf.so")
-SOURCES = ["ctsf_api.cu", "geom.cpp", "sf_bp.cu", "sf_fp.cu", "sf_filter.cu", "peak_fma.cu"]
+SOURCES = ["ctsf_api.cu", "geom.cpp", "sf_bp.cu", "sf_fp.cu", "sf_fp_noalloc.cu", "sf_filter.cu", "peak_fma.cu"]
 HEADERS = ["ctsf_internal.h", "sf_params.h", "sf_footprint.cuh", os.path.join("..", "..", "include", "ctsf.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--cudart", "static"]
