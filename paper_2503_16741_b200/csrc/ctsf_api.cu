@@ -128,6 +128,7 @@ CTSF_API int ctsf_debug_set(const char *name, double value)
     else if (n == "bp_tma") d.bp_tma = (int)value;
     else if (n == "bp_chunk") d.bp_chunk = (int)value;
     else if (n == "bp_scalar") d.bp_scalar = (int)value;
+    else if (n == "bp_poison") d.bp_poison = (int)value;
     else if (n == "host_fp_chunks") d.host_fp_chunks = (int)value;
     else if (n == "host_bp_chunks") d.host_bp_chunks = (int)value;
     else return -1;

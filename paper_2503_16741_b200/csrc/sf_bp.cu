@@ -437,7 +437,7 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
 //      FFMA2 / FMUL2 / FADD2 instructions of sm_100 (sf_footprint.cuh, "Packed pairs"): the kernel is bound by
 //      instruction issue, and the packed forms carry two voxels' multiply-adds in one issue slot.  The column and
 //      row loops run over max(K_a, K_b) x max(L_a, L_b); each footprint is cut at its own last cell edges, so the
-//      cells past them weigh exactly 0 (their loads stay inside the CTA's shared memory);
+//      cells past them weigh exactly 0 and their loads stay inside the stage's own tile and zero rows (see "parked");
 //  (2) the views flow through a ring of BP2_STAGES tile buffers guarded by mbarrier pairs: full[s] completes when
 //      the TMA bytes of the view have landed (one warp, in rotation, stages the view's parameters and the brick's
 //      shadow and arms it), empty[s] when all warps have finished reading the stage.  No __syncthreads in the view loop: warps
@@ -464,7 +464,7 @@ template <int ARC, int RECON, int MODEL>
 __global__ void __launch_bounds__(BRICK_THREADS, BP2_MINB)
 bp_brick2_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__restrict__ proj,
                  const __grid_constant__ CUtensorMap tmap, float *__restrict__ vol,
-                 int view_begin, int view_stride, int view_count, int j_lo, int j_hi, int nbz, int accumulate)
+                 int view_begin, int view_stride, int view_count, int j_lo, int j_hi, int nbz, int accumulate, int poison)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float *tiles = reinterpret_cast<float *>(smem_raw);                                    // [BP2_STAGES][TILE_FLOATS]
@@ -487,6 +487,14 @@ bp_brick2_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__
     for (int i = tid; i < (BZ / 2) * BRICK_THREADS; i += BRICK_THREADS) accs[i] = make_float2(0.0f, 0.0f);
     for (int i = tid; i < BP2_STAGES * LM * TW; i += BRICK_THREADS)
         tiles[(i / (LM * TW)) * TILE_FLOATS + TH * TW + i % (LM * TW)] = 0.0f;
+    if (poison) {
+        // testing aid (CtsfDebug::bp_poison): the data rows of every ring stage start as NaN, the worst that
+        // uninitialised shared memory can hold; a stage that no view is staged into keeps them.  No load that feeds a
+        // result may ever reach such a stage (a weight of exactly 0 does not help: 0 * NaN = NaN).
+        for (int i = tid; i < BP2_STAGES * TH * TW; i += BRICK_THREADS)
+            tiles[(i / (TH * TW)) * TILE_FLOATS + i % (TH * TW)] = __int_as_float(0x7fc00000);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // ordered before the TMA writes that follow
+    }
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < BP2_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], BRICK_THREADS / 32); }
@@ -601,10 +609,20 @@ bp_brick2_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__
                         float2 sum = p2s(0.0f);
                         const uint32_t baseA = tile_a + 4u * (unsigned)((lloA - tl0) * TW + (kloA - tk0));
                         const uint32_t baseB = tile_a + 4u * (unsigned)((lloB - tl0) * TW + (kloB - tk0));
+                        // Both voxels walk max(L_a, L_b) rows and max(K_a, K_b) columns from their own first cell.  The
+                        // one whose footprint ends first (cut by the box or the detector) would run on past the LM zero
+                        // rows below the tile -- into the next ring stage or the accumulators, which may hold anything,
+                        // and 0 * NaN is NaN.  A row chunk that would start at or below row TH (all of its rows weigh 0
+                        // for that voxel) is PARKED on the zero rows at column 0 instead: K_max <= TW columns from there
+                        // stay inside them.  With 0 <= column < TW, "row >= TH" is "address >= first zero row", so one
+                        // min does it.  A chunk that starts inside the tile ends at row TH + 2 at most, and its columns
+                        // past TW wrap into the next row of the same tile.
+                        const uint32_t zero_rows = tile_a + 4u * (unsigned)(TH * TW);
                         for (int lb = 0; lb < Lmax; lb += LM) {
                             float2 f2[LM];
                             sf_F2_run2<LM>(A, p2((float)(lloA + lb), (float)(lloB + lb)), f2);
-                            uint32_t ra = baseA + 4u * (unsigned)(lb * TW), rb = baseB + 4u * (unsigned)(lb * TW);
+                            uint32_t ra = min(baseA + 4u * (unsigned)(lb * TW), zero_rows);
+                            uint32_t rb = min(baseB + 4u * (unsigned)(lb * TW), zero_rows);
                             float2 xi = xi0, g0 = g00;
 #pragma unroll 1
                             for (int k = 0; k < Kmax; ++k, ra += 4, rb += 4) {
@@ -720,7 +738,7 @@ int launch_brick(const ct_geom *g, const float *d_proj, float *d_vol, int batch,
             // the tensor map addresses view (batch*vc + j): pass the buffer of image b0 by offsetting batch in-kernel
             if (packed && b0 == 0)
                 kern2<<<grid, BRICK_THREADS, smem2, st>>>(pr, g->d_bp, d_proj, tmap, d_vol, vb, vs, vc, j_lo, j_hi, nbz,
-                                                          accumulate || j_lo > 0);
+                                                          accumulate || j_lo > 0, g_ctsf_debug.bp_poison ? 1 : 0);
             else
                 kern<<<grid, BRICK_THREADS, smem, st>>>(pr, g->d_bp, d_proj + (size_t)b0 * vc * pr.nv * pr.nu, tmap, b0 == 0 ? use_tma : 0,
                                                         d_vol + (size_t)b0 * pr.nx * pr.ny * pr.nz, vb, vs, vc, j_lo, j_hi, nbz,

@@ -273,6 +273,31 @@ def test_backprojector_alternate_staging_and_chunking(env, monkeypatch):
     geom.close()
 
 
+@pytest.mark.parametrize("index, chunk", [(2, 1), (2, 2), (4, 1)])
+def test_packed_backprojector_never_reads_unstaged_shared_memory(index, chunk):
+    """The two voxels of a z-pair walk max(L_a, L_b) x max(K_a, K_b) cells each; the one whose footprint is cut by the
+    end of a TMA box or of the detector must not run past the tile's zero rows into the next ring stage (its weights
+    there are exactly 0, but 0 * NaN = NaN).  Footprints of ~20 rows in shadows of several boxes, one or two views
+    per launch so that one or two ring stages are never staged, those stages pre-filled with NaN (bp_poison): the
+    result must be finite and bit-identical to the unpoisoned run."""
+    from paper_2503_16741_b200.projector import Geometry
+    c = W.make_config(index, nx=24, ny=22, nz=20, nu=320, nv=300, n_views=7)
+    geom = Geometry(W.geom_keys(c))
+    rng = np.random.default_rng(31 + index)
+    y = torch.from_numpy(rng.uniform(0.5, 1.5, (1, 7, 300, 320)).astype(np.float32)).cuda()
+    B.debug_set("bp_chunk", chunk)
+    x_plain = geom.bp(y)
+    torch.cuda.synchronize()
+    B.debug_set("bp_poison", 1)
+    x_poison = geom.bp(y)
+    torch.cuda.synchronize()
+    B.debug_set("reset")
+    assert bool(torch.isfinite(x_poison).all()), "%d non-finite voxels" % int((~torch.isfinite(x_poison)).sum())
+    assert torch.equal(x_poison, x_plain)
+    assert x_plain.max().item() > 0.0
+    geom.close()
+
+
 def test_backward_direction_module_gradient_is_forward_projection():
     """"forward projection and backprojection are gradients of each other".  For the module in
     direction 'backward' (x = A^T y) autograd's gradient of <w, A^T y> with respect to y must be A w."""
