@@ -417,6 +417,11 @@ bp_brick_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__r
                         }
                     }
                 }
+            // This view's tile buffer may have been written by cp.async (generic proxy); the next write into it is
+            // warp 0's TMA (async proxy) two views on, ordered behind these writes only by the barrier below.  Writes
+            // of one proxy followed by writes of the other need a proxy fence by the writing threads.
+            if ((use_tma & 1) && (t.nbk * t.nbl > 1 || !(use_tma & 2)))
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         }
         __syncthreads();
     }
@@ -642,6 +647,9 @@ bp_brick2_kernel(SfProblem pr, const SfView *__restrict__ views, const float *__
                         *ap = p2fma(amp, sum, *ap);
                     }
                 }
+            // extra boxes were staged into this slot by cp.async (generic proxy); the slot's next writer is a TMA (async
+            // proxy) issued after empty[s] completes: every writing thread fences across the proxies before it arrives
+            if (t.nbk * t.nbl > 1) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[s]);
