@@ -15,7 +15,10 @@
  *    [batch][n_views][nv][nu], u fastest (batch = B*C flattened);
  *  - outputs are OVERWRITTEN (y = A x, x = A^T y), never accumulated into;
  *  - device entry points are asynchronous on `stream`: no host synchronisation, no host<->device
- *    copy of image data; scratch memory, when needed, comes from the stream-ordered allocator;
+ *    copy of image data.  Scratch memory: ct_fp_sf keeps its one scratch buffer in the geometry (a synchronising
+ *    cudaMalloc the first time a geometry, a larger batch or a second concurrent stream needs it, none afterwards);
+ *    ct_fp_sf_noalloc never allocates; the *_host entry points take their device buffers from the library's
+ *    stream-ordered pool; no other entry point uses scratch memory;
  *  - every function returns a ct_status_t; nothing throws across the boundary;
  *  - inputs are expected to be finite: the kernels multiply cells just outside a footprint by a weight that is
  *    exactly 0 instead of skipping them, so a NaN / Inf in the input may reach outputs up to one footprint width
@@ -94,7 +97,8 @@ CTSF_API ct_status_t ct_geom_destroy(ct_geom_t *geom);
  * Both caller-owned, fp32-aligned, must not overlap (a 16-byte aligned projection buffer with nu % 4 == 0 lets the
  * backprojector stage its tiles by TMA; other buffers take the cp.async path -- same results).  Asynchronous on
  * `stream`; makes no allocator call once the geometry is warm (the scratch for the xy-transposed volume that views
- * along x read is owned by the geometry, grown on first use and kept until ct_geom_destroy). */
+ * along x read is owned by the geometry, grown on first use and kept until ct_geom_destroy; calls in flight on
+ * different streams or from different host threads each get a buffer of their own). */
 CTSF_API ct_status_t ct_fp_sf(const ct_geom_t *geom, const float *d_vol, float *d_proj,
                      int32_t batch, ct_stream_t stream);
 

@@ -84,29 +84,46 @@ CtsfDebug g_ctsf_debug;
 void *ctsf_scratch_acquire(const ct_geom *g, size_t bytes, void *stream)
 {
     std::lock_guard<std::mutex> lock(g->scratch_mu);
+    // A slot between acquire and release belongs to the call that took it: host threads working on the same geometry
+    // never see it as free (its event says nothing yet -- never recorded, or recorded behind an EARLIER use).
+    // An idle slot is free for this call if its last use was on the same stream (stream order) or has completed.
+    ct_geom::Scratch *small = nullptr;
     for (auto &sc : g->scratch) {
-        if (sc.bytes < bytes || !sc.ptr) continue;
-        // free for this call: same stream (ordered behind the previous use), or the previous use has completed
-        if (sc.stream == stream || (sc.done && cudaEventQuery((cudaEvent_t)sc.done) == cudaSuccess)) {
-            sc.stream = stream;
-            return sc.ptr;
-        }
+        if (sc.busy || !sc.ptr) continue;
+        const bool idle = sc.stream == stream || (sc.done && cudaEventQuery((cudaEvent_t)sc.done) == cudaSuccess);
+        if (!idle) continue;
+        if (sc.bytes >= bytes) { sc.stream = stream; sc.busy = true; cudaGetLastError(); return sc.ptr; }
+        if (!small) small = &sc;
     }
     cudaGetLastError();                     // cudaEventQuery's cudaErrorNotReady is not an error here
+    void *ptr = nullptr;
+    if (small) {
+        // an idle slot that is too small (a larger batch than before) is replaced, not kept beside the new one: the
+        // geometry's scratch does not grow with every batch size it has seen.  cudaFree waits for pending work on it.
+        cudaFree(small->ptr);
+        small->ptr = nullptr; small->bytes = 0;
+        if (cudaMalloc(&ptr, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        small->ptr = ptr; small->bytes = bytes; small->stream = stream; small->busy = true;
+        return ptr;
+    }
     ct_geom::Scratch sc;
-    if (cudaMalloc(&sc.ptr, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    if (cudaMalloc(&ptr, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
     cudaEvent_t ev = nullptr;
-    if (cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); cudaFree(sc.ptr); return nullptr; }
-    sc.bytes = bytes; sc.stream = stream; sc.done = ev;
+    if (cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); cudaFree(ptr); return nullptr; }
+    sc.ptr = ptr; sc.bytes = bytes; sc.stream = stream; sc.done = ev; sc.busy = true;
     g->scratch.push_back(sc);
-    return sc.ptr;
+    return ptr;
 }
 
 void ctsf_scratch_release(const ct_geom *g, void *ptr, void *stream)
 {
     std::lock_guard<std::mutex> lock(g->scratch_mu);
     for (auto &sc : g->scratch)
-        if (sc.ptr == ptr) { cudaEventRecord((cudaEvent_t)sc.done, (cudaStream_t)stream); return; }
+        if (sc.ptr == ptr) {
+            cudaEventRecord((cudaEvent_t)sc.done, (cudaStream_t)stream);     // before the slot can be seen as idle
+            sc.busy = false;
+            return;
+        }
 }
 
 extern "C" {

@@ -23,8 +23,10 @@ struct ct_geom {
     // ct_fp_sf makes no allocator call ("any workspace is allocated in ct_geom_create" -- its size
     // depends on the batch, so it is grown on first use and kept).  A slot is reused by a later call on the same
     // stream at once (stream order), by a call on another stream only after the event recorded behind its last
-    // use has completed; otherwise another slot is made.  Freed by ct_geom_destroy.
-    struct Scratch { void *ptr = nullptr; size_t bytes = 0; void *stream = nullptr; void *done = nullptr; };
+    // use has completed; otherwise another slot is made.  `busy`: taken by a call that has not released it yet (its
+    // event is not recorded yet, so it must not be judged by it).  An idle slot that is too small for a later, larger
+    // batch is replaced by the larger buffer.  Freed by ct_geom_destroy.
+    struct Scratch { void *ptr = nullptr; size_t bytes = 0; void *stream = nullptr; void *done = nullptr; bool busy = false; };
     mutable std::vector<Scratch> scratch;
     mutable std::mutex scratch_mu;
     // host-buffer entry points: copy stream and chunk events, made on first use

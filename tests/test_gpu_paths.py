@@ -426,9 +426,9 @@ def test_forward_projector_scratch_is_reused():
     geom = Geometry(W.geom_keys(c))
     x = torch.from_numpy(W.make_phantom(c)).cuda()
     y = geom.fp(x)
+    out = torch.empty_like(y)                   # before the reading: in a fresh process torch allocates a block for it
     torch.cuda.synchronize()
     free0 = torch.cuda.mem_get_info()[0]
-    out = torch.empty_like(y)
     for _ in range(9):
         geom.fp(x, out=out)
     torch.cuda.synchronize()
@@ -445,6 +445,36 @@ def test_forward_projector_scratch_is_reused():
             geom.fp(x2, out=o2)
     torch.cuda.synchronize()
     assert torch.equal(o1, y) and torch.equal(o2, geom.fp(x2))
+    geom.close()
+
+
+def test_forward_projector_scratch_does_not_grow_with_every_batch_size():
+    """A larger batch replaces the geometry's idle scratch buffer instead of keeping the old one beside a new one:
+    after batch 1 then batch 2 the geometry holds ONE buffer of two volumes (6 MiB each), not three volumes."""
+    from paper_2503_16741_b200.projector import Geometry
+    c = W.make_config(4, nx=128, ny=128, nz=96, nu=64, nv=48, n_views=8)
+    geom = Geometry(W.geom_keys(c))
+    vol_bytes = 128 * 128 * 96 * 4
+    x2 = torch.rand((2, 96, 128, 128), device="cuda")
+    out1 = torch.empty((1, 8, 48, 64), device="cuda")
+    out2 = torch.empty((2, 8, 48, 64), device="cuda")
+    warm = Geometry(W.geom_keys(c))               # first launches load the kernels (device memory of their own)
+    warm.fp(x2, out=out2)
+    torch.cuda.synchronize()
+    warm.close()
+    free_cold = torch.cuda.mem_get_info()[0]
+    geom.fp(x2[:1], out=out1)
+    torch.cuda.synchronize()
+    free_b1 = torch.cuda.mem_get_info()[0]
+    geom.fp(x2, out=out2)
+    torch.cuda.synchronize()
+    free_b2 = torch.cuda.mem_get_info()[0]
+    assert free_cold - free_b1 >= vol_bytes                      # this geometry does use the scratch
+    assert free_cold - free_b2 <= 2 * vol_bytes + (2 << 20), (free_cold - free_b1, free_cold - free_b2)
+    assert torch.equal(out2[:1], out1)
+    geom.fp(x2[:1], out=out1)                                    # the larger buffer serves the smaller batch
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free_b2
     geom.close()
 
 
