@@ -45,54 +45,54 @@ class Geometry:
     def fp(self, vol, views=None, out=None):
         """vol [..., nz, ny, nx] -> proj [..., n_sel, nv, nu]."""
         vb, vs, vc = self._views(views)
-        lead, batch, vol = _prep(vol, self.vol_shape, -3 if self.dim == 2 else None)
+        lead, batch, vol, sq = _prep(vol, self.vol_shape, -3 if self.dim == 2 else None)
         out = _out(out, (batch, vc) + self.det_shape, vol.device)
         B.ct_fp_sf_views(self.handle, vol.data_ptr(), out.data_ptr(), batch, vb, vs, vc,
                          torch.cuda.current_stream(vol.device).cuda_stream)
-        return out.view(lead + self._tail((vc,) + self.det_shape, -2, vol))
+        return out.view(lead + self._tail((vc,) + self.det_shape, -2, sq))
 
     def bp(self, proj, views=None, out=None):
         """proj [..., n_sel, nv, nu] -> vol [..., nz, ny, nx]."""
         vb, vs, vc = self._views(views)
-        lead, batch, proj = _prep(proj, (vc,) + self.det_shape, -2 if self.dim == 2 else None)
+        lead, batch, proj, sq = _prep(proj, (vc,) + self.det_shape, -2 if self.dim == 2 else None)
         out = _out(out, (batch,) + self.vol_shape, proj.device)
         B.ct_bp_sf_views(self.handle, proj.data_ptr(), out.data_ptr(), batch, vb, vs, vc,
                          torch.cuda.current_stream(proj.device).cuda_stream)
-        return out.view(lead + self._tail(self.vol_shape, -3, proj))
+        return out.view(lead + self._tail(self.vol_shape, -3, sq))
 
     # ---- recon mode (PAPER.md:103, 68; DESIGN.md readings R23, R24) --------------------------------
     def fbp_filter(self, proj, views=None, out=None):
         """Cosine pre-weight + discrete ramp filter along the channels; proj [..., n_sel, nv, nu] -> same shape."""
         vb, vs, vc = self._views(views)
-        lead, batch, proj = _prep(proj, (vc,) + self.det_shape, -2 if self.dim == 2 else None)
+        lead, batch, proj, sq = _prep(proj, (vc,) + self.det_shape, -2 if self.dim == 2 else None)
         out = _out(out, tuple(proj.shape), proj.device)
         B.ct_fbp_filter_views(self.handle, proj.data_ptr(), out.data_ptr(), batch, vb, vs, vc,
                               torch.cuda.current_stream(proj.device).cuda_stream)
-        return out.view(lead + self._tail((vc,) + self.det_shape, -2, proj))
+        return out.view(lead + self._tail((vc,) + self.det_shape, -2, sq))
 
     def bp_recon(self, proj, views=None, out=None):
         """Recon-mode backprojection (normalised footprints x depth weight); proj [..., n_sel, nv, nu] -> volume."""
         vb, vs, vc = self._views(views)
-        lead, batch, proj = _prep(proj, (vc,) + self.det_shape, -2 if self.dim == 2 else None)
+        lead, batch, proj, sq = _prep(proj, (vc,) + self.det_shape, -2 if self.dim == 2 else None)
         out = _out(out, (batch,) + self.vol_shape, proj.device)
         B.ct_bp_sf_recon_views(self.handle, proj.data_ptr(), out.data_ptr(), batch, vb, vs, vc,
                                torch.cuda.current_stream(proj.device).cuda_stream)
-        return out.view(lead + self._tail(self.vol_shape, -3, proj))
+        return out.view(lead + self._tail(self.vol_shape, -3, sq))
 
     def fbp(self, proj, out=None):
         """Filtered backprojection of N equi-angular views over 360 degrees: (pi / N) B(filter(p)) (ct_fbp_sf)."""
-        lead, batch, proj = _prep(proj, (self.n_views,) + self.det_shape, -2 if self.dim == 2 else None)
+        lead, batch, proj, sq = _prep(proj, (self.n_views,) + self.det_shape, -2 if self.dim == 2 else None)
         out = _out(out, (batch,) + self.vol_shape, proj.device)
         work = torch.empty_like(proj)
         B.ct_fbp_sf(self.handle, proj.data_ptr(), work.data_ptr(), out.data_ptr(), batch,
                     torch.cuda.current_stream(proj.device).cuda_stream)
-        return out.view(lead + self._tail(self.vol_shape, -3, proj))
+        return out.view(lead + self._tail(self.vol_shape, -3, sq))
 
-    def _tail(self, tail, unit_axis, like):
+    def _tail(self, tail, unit_axis, squeezed):
         """Output tail shape: 2-D inputs given without their unit axis ([..., ny, nx] / [..., views, nu], the paper's
-        own usage) get outputs without theirs too."""
+        own usage; `squeezed` as reported by _prep) get outputs without theirs too."""
         tail = tuple(tail)
-        if self.dim == 2 and getattr(like, "_ctsf_squeezed", False):
+        if self.dim == 2 and squeezed:
             i = len(tail) + unit_axis
             return tail[:i] + tail[i + 1:]
         return tail
@@ -120,23 +120,28 @@ class Geometry:
 
 
 def _prep(t, tail, unit_axis=None):
-    """Contiguous fp32 view [batch, *tail] of a CUDA tensor whose trailing dims are `tail`.  unit_axis (2-D geometries):
-    index in `tail` of the unit z / row axis, which may be missing: [..., ny, nx] and [..., views, nu] are accepted."""
+    """(lead, batch, view, squeezed): the contiguous fp32 view [batch, *tail] of a CUDA tensor whose trailing dims are
+    `tail`, the leading dims it had, and whether the unit axis was missing.  unit_axis (2-D geometries): index in `tail`
+    of the unit z / row axis, which may be left out: [..., ny, nx] and [..., views, nu] are accepted.
+    One shape reads both ways -- a rank-3 [1, ny, nx] is "one image with its unit z axis" and "a batch of one image
+    without it".  Rank decides, never the batch size: a tensor of exactly len(tail) dims given to a 2-D geometry is
+    [batch, ny, nx] (so the last mini-batch of a loop, of size 1, comes back as [1, views, nu] like its predecessors
+    came back as [B, views, nu]); the unit axis counts from rank len(tail) + 1 on ([B, 1, ny, nx])."""
     if not t.is_cuda:
         raise RuntimeError("ctsf operators take CUDA tensors (no CPU fallback)")
     if t.dtype != torch.float32:
         raise TypeError("ctsf operators compute in float32; got %s (cast explicitly)" % t.dtype)
     tail = tuple(tail)
     nd = len(tail)
-    squeezed = False
-    if tuple(t.shape[-nd:]) != tail:
-        i = nd + unit_axis if unit_axis is not None else None
-        short = tail[:i] + tail[i + 1:] if i is not None else None
-        if short is not None and tail[i] == 1 and tuple(t.shape[-(nd - 1):]) == short:
-            t = t.unsqueeze(t.dim() - (nd - 1) + i)
-            squeezed = True
-        else:
-            raise ValueError("expected trailing shape %s, got %s" % (tail, tuple(t.shape)))
+    full = t.dim() >= nd and tuple(t.shape[-nd:]) == tail
+    i = nd + unit_axis if unit_axis is not None else None
+    short = tail[:i] + tail[i + 1:] if i is not None and tail[i] == 1 else None
+    squeezed = short is not None and t.dim() >= nd - 1 and tuple(t.shape[-(nd - 1):]) == short and \
+        (not full or t.dim() == nd)
+    if squeezed:
+        t = t.unsqueeze(t.dim() - (nd - 1) + i)
+    elif not full:
+        raise ValueError("expected trailing shape %s, got %s" % (tail, tuple(t.shape)))
     lead = tuple(t.shape[:-nd])
     t = t.detach().contiguous()
     batch = 1
@@ -144,9 +149,7 @@ def _prep(t, tail, unit_axis=None):
         batch *= s
     if batch < 1:
         raise ValueError("empty batch")
-    t = t.view((batch,) + tail)
-    t._ctsf_squeezed = squeezed
-    return lead, batch, t
+    return lead, batch, t.view((batch,) + tail), squeezed
 
 
 def _out(out, shape, device):
