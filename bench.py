@@ -199,6 +199,7 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
+    B.debug_set("reset")                               # the library's testing switches: every one at its default
     g = dict(W.geom_keys(c), algo=args.algo)
     x_host = W.make_phantom(c)                         # [B, nz, ny, nx] fp32, seeded
     batch = c["batch"]
@@ -360,6 +361,7 @@ def main():
             "fp_ms": fp_ms, "bp_ms": bp_ms,
             "fp_gups": updates / (fp_ms * 1e-3) / 1e9, "bp_gups": updates / (bp_ms * 1e-3) / 1e9,
             "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "recon": recon,
+            "debug_switches": B.debug_state(),       # testing switches off their defaults after the run: {} expected
             "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak,
                          "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
                          "peak_src": "measured in this run by ct_measure_fp32_peak (FMA-only kernel, best of 2 x 3): "

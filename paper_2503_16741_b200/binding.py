@@ -66,6 +66,8 @@ def lib():
         L.ct_fbp_sf.argtypes = [P, P, P, P, I, P]
         L.ctsf_debug_set.argtypes = [ctypes.c_char_p, ctypes.c_double]
         L.ctsf_debug_set.restype = ctypes.c_int
+        L.ctsf_debug_get.argtypes = [ctypes.c_char_p]
+        L.ctsf_debug_get.restype = ctypes.c_double
         L.ct_measure_fp32_peak.argtypes = [I, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), P]
         L.ct_last_launch_count.argtypes = [P]
         L.ct_last_launch_count.restype = I
@@ -183,6 +185,23 @@ def debug_set(name, value=1):
     debug_set('reset') restores the defaults.  Used by tests only."""
     if lib().ctsf_debug_set(name.encode(), float(value)) != 0:
         raise KeyError(name)
+
+
+DEBUG_DEFAULTS = {"fp_pad": 0.0, "tt_pad": 0.0, "fp_nohoist": 0, "fp_forcehoist": 0, "fp_serial": 0, "bp_nohoist": 0,
+                  "bp_forcehoist": 0, "bp_tma": -1, "bp_chunk": 0, "bp_scalar": 0, "bp_poison": 0,
+                  "host_fp_chunks": 0, "host_bp_chunks": 0}
+
+
+def debug_state():
+    """The testing switches that are NOT at their defaults, as {name: value} (ctsf_debug_get); {} = product paths."""
+    out = {}
+    for name, default in DEBUG_DEFAULTS.items():
+        v = lib().ctsf_debug_get(name.encode())
+        if v != v:
+            raise KeyError(name)
+        if v != default:
+            out[name] = v
+    return out
 
 
 def ct_measure_fp32_peak(kind=0, stream=0):

@@ -128,28 +128,46 @@ void ctsf_scratch_release(const ct_geom *g, void *ptr, void *stream)
 
 extern "C" {
 
-// Testing aid, deliberately NOT declared in include/ctsf.h: sets one switch of CtsfDebug by name (see ctsf_internal.h).
-// Returns 0, or -1 for an unknown name.  Not thread-safe against running calls.
+// Testing aids, deliberately NOT declared in include/ctsf.h.  ctsf_debug_set sets one switch of CtsfDebug by name (see
+// ctsf_internal.h; "reset" restores every default) and returns 0, or -1 for an unknown name.  ctsf_debug_get returns
+// the switch's current value, NaN for an unknown name: bench.py records with it that it timed the default paths.
+// Process-wide and not thread-safe against running calls: for tests only.
+static int debug_field(CtsfDebug &d, const std::string &n, float **f, int **i)
+{
+    *f = nullptr; *i = nullptr;
+    if (n == "fp_pad") *f = &d.fp_pad;
+    else if (n == "tt_pad") *f = &d.tt_pad;
+    else if (n == "fp_nohoist") *i = &d.fp_nohoist;
+    else if (n == "fp_forcehoist") *i = &d.fp_forcehoist;
+    else if (n == "fp_serial") *i = &d.fp_serial;
+    else if (n == "bp_nohoist") *i = &d.bp_nohoist;
+    else if (n == "bp_forcehoist") *i = &d.bp_forcehoist;
+    else if (n == "bp_tma") *i = &d.bp_tma;
+    else if (n == "bp_chunk") *i = &d.bp_chunk;
+    else if (n == "bp_scalar") *i = &d.bp_scalar;
+    else if (n == "bp_poison") *i = &d.bp_poison;
+    else if (n == "host_fp_chunks") *i = &d.host_fp_chunks;
+    else if (n == "host_bp_chunks") *i = &d.host_bp_chunks;
+    else return -1;
+    return 0;
+}
+
 CTSF_API int ctsf_debug_set(const char *name, double value)
 {
     if (!name) return -1;
     const std::string n(name);
-    CtsfDebug &d = g_ctsf_debug;
-    if (n == "reset") d = CtsfDebug();
-    else if (n == "fp_pad") d.fp_pad = (float)value;
-    else if (n == "fp_nohoist") d.fp_nohoist = (int)value;
-    else if (n == "fp_forcehoist") d.fp_forcehoist = (int)value;
-    else if (n == "fp_serial") d.fp_serial = (int)value;
-    else if (n == "bp_nohoist") d.bp_nohoist = (int)value;
-    else if (n == "bp_forcehoist") d.bp_forcehoist = (int)value;
-    else if (n == "bp_tma") d.bp_tma = (int)value;
-    else if (n == "bp_chunk") d.bp_chunk = (int)value;
-    else if (n == "bp_scalar") d.bp_scalar = (int)value;
-    else if (n == "bp_poison") d.bp_poison = (int)value;
-    else if (n == "host_fp_chunks") d.host_fp_chunks = (int)value;
-    else if (n == "host_bp_chunks") d.host_bp_chunks = (int)value;
-    else return -1;
+    if (n == "reset") { g_ctsf_debug = CtsfDebug(); return 0; }
+    float *f; int *i;
+    if (debug_field(g_ctsf_debug, n, &f, &i) != 0) return -1;
+    if (f) *f = (float)value; else *i = (int)value;
     return 0;
+}
+
+CTSF_API double ctsf_debug_get(const char *name)
+{
+    float *f; int *i;
+    if (!name || debug_field(g_ctsf_debug, std::string(name), &f, &i) != 0) return std::nan("");
+    return f ? (double)*f : (double)*i;
 }
 
 ct_status_t ct_geom_create(const ct_geom_desc_t *d, ct_geom_t **out)

@@ -51,6 +51,7 @@ struct CtsfDebug {
     int bp_chunk = 0;             // views per backprojector launch (0: sized for L2)
     int bp_scalar = 0;            // general frames: one voxel per thread (the round-1 kernel) instead of packed pairs
     int bp_poison = 0;            // packed backprojector: ring stages start as NaN (no load may reach an unstaged one)
+    float tt_pad = 0.0f;          // SF-TT: rows / voxels added to the sampled trapezoid margins (lpad, zpad) at ct_geom_create
     int host_fp_chunks = 0;       // host-buffer A / A^T: number of view chunks of the copy/compute pipeline (0: default)
     int host_bp_chunks = 0;
 };

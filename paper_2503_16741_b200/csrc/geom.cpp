@@ -203,8 +203,11 @@ ct_status_t ctsf_build_views(const ct_geom_desc_t *d, ct_geom *g)
             o.lane_stride = std::max(stride, 1);
             o.ek = (float)(hk_max * 1.10 + 0.05);
             o.el = (float)(is3 ? hl_max * 1.10 + 0.05 : 0.0);
-            o.lpad = (float)(d->algo == CT_ALGO_SFTT && is3 ? lpad_max * 1.25 + 0.1 : 0.0);
-            o.zpad = (float)(d->algo == CT_ALGO_SFTT && is3 ? zpad_max * 1.25 + 0.1 : 0.0);
+            // testing aid (CtsfDebug::tt_pad, read when the geometry is created): extra rows / voxels on top of the
+            // sampled SF-TT margins -- a result that changes with it beyond summation order means they were too small
+            const double tt_pad = g_ctsf_debug.tt_pad;
+            o.lpad = (float)(d->algo == CT_ALGO_SFTT && is3 ? lpad_max * 1.25 + 0.1 + tt_pad : 0.0);
+            o.zpad = (float)(d->algo == CT_ALGO_SFTT && is3 ? zpad_max * 1.25 + 0.1 + tt_pad : 0.0);
             g->h_bp[i].lpad = o.lpad;                  // the backprojector's brick shadow uses the same margin
             // columns / rows one footprint can span: floor(kc+t3) - floor(kc+t0) + 1 <= 2 ek + 2
             if (2.0 * o.ek + 2.0 > 6.0 || 2.0 * o.el + 2.0 > 8.0) small_fp = 0;

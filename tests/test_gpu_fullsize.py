@@ -60,7 +60,81 @@ def test_parity_full_size_sampled(index):
     geom.close()
 
 
-@pytest.mark.parametrize("algo", ["SF", "DD"])
+def test_sftt_full_size_sampled():
+    """SF-TT (row f3) at config 4's full size: A on whole sampled views, A^T on sampled voxels over all 720 views,
+    against the oracle's algo='SF-TT' -- the sizes at which its sampled margins (lpad, zpad) have to hold."""
+    from paper_2503_16741_b200.projector import Geometry
+    c = W.make_config(4)
+    g = dict(W.geom_keys(c), algo="SF-TT")
+    o = Oracle(g)
+    rng = np.random.default_rng(9400)
+    x = W.make_phantom(c)
+    geom = Geometry(g)
+    xd = torch.from_numpy(x).cuda()
+    y = geom.fp(xd)
+    views = np.sort(rng.choice(c["n_views"], 4, replace=False))
+    y_ref = o.fp(x, views)
+    y_gpu = y[:, torch.from_numpy(views).cuda()].double().cpu().numpy()
+    rel = np.linalg.norm(y_gpu - y_ref) / np.linalg.norm(y_ref)
+    mx = np.abs(y_gpu - y_ref).max() / np.abs(y_ref).max()
+    assert rel <= 1e-5 and mx <= 1e-4, "SF-TT A config 4: rel-L2 %.3e max %.3e" % (rel, mx)
+    del y, xd
+    p = W.make_projections(c)
+    xb = geom.bp(torch.from_numpy(p).cuda())
+    n = 2000
+    ijk = np.stack([rng.integers(0, c["nx"], n), rng.integers(0, c["ny"], n), rng.integers(0, c["nz"], n)], axis=1)
+    ijk[0] = (0, 0, 0)
+    ijk[1] = (c["nx"] - 1, c["ny"] - 1, c["nz"] - 1)
+    ref = o.bp_voxels(p[0], ijk)
+    got = xb[0, ijk[:, 2], ijk[:, 1], ijk[:, 0]].double().cpu().numpy()
+    rel = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+    mx = np.abs(got - ref).max() / np.abs(ref).max()
+    assert rel <= 1e-5 and mx <= 1e-4, "SF-TT A^T config 4: rel-L2 %.3e max %.3e" % (rel, mx)
+    geom.close()
+
+
+def test_sftt_margins_are_conservative_full_size():
+    """SF-TT's trapezoid reaches beyond the rectangle's rows; how far is SAMPLED when the geometry is created (a 9x9x9
+    probe x 1.25: lpad for the backprojector's brick shadow, zpad for the forward kernel's region).  Nothing re-checks
+    it at run time, so it is checked here where it matters: at config 4's full volume and detector (96 of its views),
+    two more rows / voxels of margin (testing switch tt_pad) may change A and A^T by summation order only."""
+    from paper_2503_16741_b200.projector import Geometry
+    c = W.make_config(4, n_views=96)
+    g = dict(W.geom_keys(c), algo="SF-TT")
+    rng = np.random.default_rng(81)
+    x = torch.from_numpy(rng.uniform(0.5, 1.5, (1, c["nz"], c["ny"], c["nx"])).astype(np.float32)).cuda()
+    y = torch.from_numpy(rng.uniform(0.5, 1.5, (1, c["n_views"], c["nv"], c["nu"])).astype(np.float32)).cuda()
+    geom = Geometry(g)
+    B.debug_set("tt_pad", 2.0)
+    wide = Geometry(g)                                  # the switch is read when the geometry is created
+    B.debug_set("tt_pad", 0.0)
+    y_t, y_w = geom.fp(x), wide.fp(x)
+    assert (y_t - y_w).abs().max().item() <= 3e-6 * y_w.abs().max().item()
+    del y_t, y_w
+    x_t, x_w = geom.bp(y), wide.bp(y)
+    assert (x_t - x_w).abs().max().item() <= 3e-6 * x_w.abs().max().item()
+    geom.close()
+    wide.close()
+
+
+def test_recon_mode_full_size_few_views():
+    """Recon mode (row f2) on config 4's full volume and detector: the RECON instantiation of the packed backprojector
+    has its own register allocation, and the shrunken configs of test_gpu_recon.py never fill a brick grid of 32^3.
+    Six of the trajectory's views, so that the oracle can backproject the WHOLE volume: every voxel is compared."""
+    from paper_2503_16741_b200.projector import Geometry
+    c = W.make_config(4, n_views=6)
+    g = W.geom_keys(c)
+    o, geom = Oracle(g), Geometry(g)
+    q = W.make_projections(c)
+    got = geom.bp_recon(torch.from_numpy(q).cuda()).double().cpu().numpy()
+    ref = o.bp_recon(q)
+    rel = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+    mx = np.abs(got - ref).max() / np.abs(ref).max()
+    assert rel <= 1e-5 and mx <= 1e-4, "recon A^T config 4, 6 views: rel-L2 %.3e max %.3e" % (rel, mx)
+    geom.close()
+
+
+@pytest.mark.parametrize("algo", ["SF", "DD", "SF-TT"])
 @pytest.mark.parametrize("index", [4, 3, 2])
 def test_forward_region_is_conservative(index, algo, monkeypatch):
     """The forward kernel sweeps, per slab, only the voxels its tile's frustum can touch (exact half-voxel halo).

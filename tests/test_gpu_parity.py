@@ -93,7 +93,10 @@ def test_edge_cases():
     g1 = W.geom_keys(c1)
     geom = Geometry(g1)
     x1 = np.ones((1, 1, 1, 1), np.float32)
-    check(geom.fp(torch.from_numpy(x1).cuda()), Oracle(g1).fp(x1), "A single voxel")
+    y1_ref = Oracle(g1).fp(x1)
+    check(geom.fp(torch.from_numpy(x1).cuda()), y1_ref, "A single voxel")
+    y1 = y1_ref.astype(np.float32)
+    check(geom.bp(torch.from_numpy(y1).cuda()), Oracle(g1).bp(y1), "A^T single voxel")
     geom.close()
     # error behaviour: bad descriptors are refused, nothing throws across the ABI
     bad = dict(g, det_u=np.array(g["det_u"]) * 1.1)

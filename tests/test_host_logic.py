@@ -35,6 +35,23 @@ def test_library_exports_every_declared_symbol():
     assert B.lib().ct_geom_destroy(None) == 0          # destroy(NULL) is CT_OK
 
 
+def test_testing_switches_round_trip():
+    """ctsf_debug_set / ctsf_debug_get (testing aids outside include/ctsf.h): every switch the binding knows exists
+    in the library with the default the binding states, set -> get round-trips, reset restores, unknown names fail."""
+    B.debug_set("reset")
+    assert B.debug_state() == {}
+    for name, default in B.DEBUG_DEFAULTS.items():
+        B.debug_set(name, 3)
+        assert B.debug_state() == {name: 3.0}
+        B.debug_set(name, default)
+    B.debug_set("bp_chunk", 5)
+    B.debug_set("reset")
+    assert B.debug_state() == {}
+    with pytest.raises(KeyError):
+        B.debug_set("no_such_switch", 1)
+    assert B.lib().ctsf_debug_get(b"no_such_switch") != B.lib().ctsf_debug_get(b"no_such_switch")     # NaN
+
+
 def test_descriptor_validation_without_gpu():
     c = W.make_config(2, nx=8, ny=8, nz=8, nu=12, nv=12, n_views=4)
     g = W.geom_keys(c)
