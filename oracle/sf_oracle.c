@@ -17,8 +17,11 @@
  * and 3-D footprints; brute-force ray/box chords; analytic disk/ellipsoid chords; mass
  * identities; parallel-beam column sums; 2-D == one-slice 3-D; dense-matrix transpose; adjoint
  * to 1e-12; symmetries; tilted frames and reversed axes against an independent ray/detector intersection model;
- * every factor of recon mode against analytic FBP/FDK; tests/test_oracle_mutations.py applies 24 one-line mutations
- * of this file and checks that a named pin fails for each.  Unpinned: nothing.
+ * every factor of recon mode against analytic FBP/FDK; the SF-TT branch (R27) hand-worked through the same independent
+ * intersection model at ~13 and ~25 degrees of polar angle, against a brute-force chord fraction, and in recon mode;
+ * the DD tie rule (R26) on an exact-tie pixel; tests/test_oracle_mutations.py applies 28 one-line mutations
+ * of this file and checks that a named pin fails for each.  Unpinned: model 3 ("SF-TT-A2", the row-dependent polar
+ * amplitude) has the relative error table of tests/test_oracle_sftt.py only -- oracle-only, no kernel uses it.
  *
  * Build: gcc -O2 -fopenmp -shared -fPIC -o libsf_oracle.so sf_oracle.c -lm
  */

@@ -38,6 +38,25 @@ def test_dd_hand_worked_2d():
     assert abs((f["tau"][2] - f["tau"][0]) - 1000.0 / 500.5) < 1e-9
 
 
+def test_dd_exact_tie_takes_the_face_across_y():
+    """R26's tie rule: when dx/|e_x| == dy/|e_y| exactly, the ray counts as running along y and the voxel is its face
+    across y, the segment x_c -+ dx/2 at y_c.  Source at (400.5, 400.5), pixel (64, 64) centred at (0.5, 0.5): e =
+    (-400, -400) in exact arithmetic.  n = -(1, 1)/sqrt(2), u = (1, -1)/sqrt(2), R = 1200: the segment's ends (0, 0.5)
+    and (1, 0.5) project to s = R b / a = 1200 (-0.5)/800.5 and 1200 (0.5)/799.5; the OTHER face, (0.5, 0) - (0.5, 1),
+    would give the mirror image, 1200 (0.5)/800.5 and 1200 (-0.5)/799.5 -- 1e-3 mm away."""
+    r2 = math.sqrt(0.5)
+    S = np.array([[400.5, 400.5, 0.0]])
+    n = np.array([-r2, -r2, 0.0])
+    g = dict(dim=2, nx=128, ny=128, nz=1, dx=1.0, dy=1.0, dz=1.0, ox=0.0, oy=0.0, oz=0.0, nu=64, nv=1, du=0.25, dv=1.0,
+             det_type="flat", src=S, det_center=S + 1200.0 * n, det_u=np.array([[r2, -r2, 0.0]]),
+             det_v=np.array([[0.0, 0.0, 1.0]]), algo="DD")
+    f = Oracle(g).footprint(0, 64, 64)
+    want = [1200.0 * -0.5 / 800.5, 1200.0 * 0.5 / 799.5]
+    assert np.allclose(f["tau"], [want[0], want[0], want[1], want[1]], atol=1e-12, rtol=0.0)
+    assert abs(want[1] + want[0]) > 9e-4                 # the two faces are distinguishable here
+    assert abs(f["amp"] - math.sqrt(2.0)) < 1e-12        # |e| dy/|e_y| = 400 sqrt(2) / 400
+
+
 def test_dd_parallel_limit_is_exact():
     """Parallel beam along y with nu = nx, du = dx: distance-driven projection is exactly dy x column sums;
     at 45 degrees with dx = dy the face model gives each pixel a rectangle of width dx/sqrt(2) and amplitude

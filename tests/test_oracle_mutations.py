@@ -85,11 +85,11 @@ MUTATIONS = {
     "recon_flat_depth_weight_uses_R_for_d": (
         "(-Sn) * f->R / (a*a)", 1, 0,
         "f->R * f->R / (a*a)",
-        [(TR.test_recon_backprojection_weights_are_normalised, {})]),
+        [(TR.test_recon_backprojection_weights_are_normalised, dict(algo="SF"))]),
     "recon_sumF1_is_the_full_base": (
         "double sumF1 = 0.5*(tau[3] + tau[2] - tau[1] - tau[0]) / g->du", 1, 0,
         "double sumF1 = (tau[3] - tau[0]) / g->du",
-        [(TR.test_recon_backprojection_weights_are_normalised, {})]),
+        [(TR.test_recon_backprojection_weights_are_normalised, dict(algo="SF"))]),
     "recon_filter_not_scaled_by_du": (
         "q[k] = g->du * acc;", 1, 0,
         "q[k] = acc;",
@@ -122,6 +122,24 @@ MUTATIONS = {
         "F2[l - llo] = (hi - lo > 0.0 ? hi - lo : 0.0) / g->dv;", 1, 0,
         "F2[l - llo] = (hi - lo > 0.0 ? hi - lo : 0.0);",
         [(T1.test_p4_golden_3d, {})]),
+    # ---- the three that survived ---------------------------------------------------------
+    "sftt_half_chord_0p4": (
+        "double P[3] = { Pc[0] + sn*0.5*lth*ux, Pc[1] + sn*0.5*lth*uy, Pc[2] + sz*0.5*g->dz };", 1, 0,
+        "double P[3] = { Pc[0] + sn*0.4*lth*ux, Pc[1] + sn*0.4*lth*uy, Pc[2] + sz*0.5*g->dz };",
+        [(T3.test_sftt_axial_profile_is_the_chord_fraction_between_the_voxel_faces, {}),
+         (T3.test_sftt_footprint_from_ray_detector_intersection, dict(det="flat"))]),
+    "sftt_recon_normalised_by_the_base": (
+        "if (sumF2_out) *sumF2_out = 0.5*(xi[3] + xi[2] - xi[1] - xi[0]) / g->dv;", 1, 0,
+        "if (sumF2_out) *sumF2_out = (xi[3] - xi[0]) / g->dv;",
+        [(TR.test_recon_backprojection_weights_are_normalised, dict(algo="SF-TT"))]),
+    "dd_tie_goes_the_other_way": (
+        "int along_y = g->dy * ex <= g->dx * ey;", 1, 0,
+        "int along_y = g->dy * ex < g->dx * ey;",
+        [(TD.test_dd_exact_tie_takes_the_face_across_y, {})]),
+    "sftt_chord_of_the_longer_axis": (
+        "double lth = rx_ < ry_ ? rx_ : ry_;", 1, 0,
+        "double lth = rx_ < ry_ ? ry_ : rx_;",
+        [(T3.test_sftt_footprint_from_ray_detector_intersection, dict(det="arc"))]),
     "backprojection_drops_the_amplitude": (
         "acc += amp * F1[k - klo] * F2[l - llo] * y[(size_t)l*g->nu + k];", 1, 0,
         "acc += F1[k - klo] * F2[l - llo] * y[(size_t)l*g->nu + k];",

@@ -82,6 +82,27 @@ def _expected_footprint(g, view, ijk):
     return np.array(tau), amp * np.outer(F2, F1)
 
 
+def _expected_footprint_tt(g, view, ijk):
+    """SF-TT weights of one voxel from reading R27 with the intersection model above: transaxial trapezoid and
+    amplitude as SF-TR; the axial factor is the unit-height trapezoid whose four vertices are the row coordinates of
+    the ends of the centre ray's in-plane chord, P_c -+ (l_theta / 2) e_xy / |e_xy|, taken at z_c - dz/2 and at
+    z_c + dz/2.  Returns (xi, area of the trapezoid in rows, weights)."""
+    Pc = _centre(g, ijk)
+    hx, hy, hz = 0.5 * g["dx"], 0.5 * g["dy"], 0.5 * g["dz"]
+    tau = sorted(_hit(g, view, Pc + np.array([sx * hx, sy * hy, 0.0]))[0] for sx in (-1, 1) for sy in (-1, 1))
+    nu, nv, du, dv = g["nu"], g["nv"], g["du"], g["dv"]
+    F1 = np.array([_trap_integral(tau, (k - 0.5 * nu) * du, (k + 1 - 0.5 * nu) * du) / du for k in range(nu)])
+    e = Pc - g["src"][view]
+    exy = e[:2] / np.hypot(e[0], e[1])
+    l_theta = min(g["dx"] / abs(exy[0]), g["dy"] / abs(exy[1]))          # in-plane chord of the centre ray
+    ends = [Pc + np.array([sn * 0.5 * l_theta * exy[0], sn * 0.5 * l_theta * exy[1], sz * hz])
+            for sn in (-1, 1) for sz in (-1, 1)]
+    xi = sorted(_hit(g, view, P)[1] for P in ends)
+    F2 = np.array([_trap_integral(xi, (l - 0.5 * nv) * dv, (l + 1 - 0.5 * nv) * dv) / dv for l in range(nv)])
+    amp = np.linalg.norm(e) * min(g["dx"] / abs(e[0]), g["dy"] / abs(e[1]))
+    return np.array(xi), 0.5 * (xi[3] + xi[2] - xi[1] - xi[0]) / dv, amp * np.outer(F2, F1)
+
+
 def _dense(f, nv, nu):
     w = np.zeros((nv, nu))
     w[f["l_lo"]:f["l_hi"] + 1, f["k_lo"]:f["k_hi"] + 1] = f["w"]
@@ -127,6 +148,72 @@ def test_tilted_frame_config4_shape():
             assert np.abs(_dense(f, g["nv"], g["nu"]) - w).max() < 1e-12
             checked += 1
     assert checked >= 8
+
+
+# ---- R27: the trapezoid axial footprint (SF-TT), hand-worked through the intersection model ------------------
+def _tt_geometry(det, algo="SF-TT"):
+    """Short orbit (SAD 200, SDD 400), tall volume (z up to +-95 mm), tilted frames (phi = +-10 deg, psi = +-0.5 deg):
+    the voxels used below see the source (itself 35 mm off the mid-plane) under polar angles of ~13 and ~25 degrees."""
+    return dict(geom3d([0.4, 2.5], det, n=(40, 40, 96), d=(2.0, 2.0, 2.0), nu=128, nv=600, du=3.0, dv=1.0,
+                       sad=200.0, sdd=400.0, phi=np.radians([10.0, -10.0]), psi=np.radians([0.5, -0.5])), algo=algo)
+
+
+TT_VOXELS = [(0, (25, 14, 40)), (1, (12, 27, 7)), (0, (12, 27, 23)), (1, (25, 14, 76))]
+
+
+@pytest.mark.parametrize("det", ["flat", "arc"])
+def test_sftt_footprint_from_ray_detector_intersection(det):
+    """Reading R27 to 1e-12: chord ends at P_c -+ (l_theta/2) e_xy/|e_xy| (a half chord of 0.4 l_theta moves the weights
+    by ~5 %), heights z_c -+ dz/2, vertices through the detector model of THIS file, trapezoid integrated piecewise.
+    The first two voxels sit at ~13 degrees of polar angle, the last two at ~25."""
+    g = _tt_geometry(det)
+    o = Oracle(g)
+    polar = []
+    for view, ijk in TT_VOXELS:
+        e = _centre(g, ijk) - g["src"][view]
+        polar.append(math.degrees(math.atan2(abs(e[2]), math.hypot(e[0], e[1]))))
+        f = o.footprint(view, *ijk)
+        xi, _, w = _expected_footprint_tt(g, view, ijk)
+        assert f is not None and 0 < f["l_lo"] and f["l_hi"] < g["nv"] - 1          # fully on the detector
+        assert np.abs(_dense(f, g["nv"], g["nu"]) - w).max() < 1e-12
+        # and it is not SF-TR's footprint: the rectangle between the rows of (x_c, y_c, z_c -+ dz/2) differs visibly
+        w_tr = _expected_footprint(g, view, ijk)[1]
+        assert np.abs(w - w_tr).max() > 0.02 * w.max(), np.abs(w - w_tr).max() / w.max()
+        assert xi[1] - xi[0] > 0.05 * (xi[3] - xi[0])                              # real ramps at these angles
+    assert 11.0 < polar[0] < 15.0 and 11.0 < polar[1] < 15.0 and 23.0 < polar[2] < 27.0 and 23.0 < polar[3] < 27.0
+
+
+def test_sftt_axial_profile_is_the_chord_fraction_between_the_voxel_faces():
+    """What R27's trapezoid stands for, by brute force, without its vertex formula: in the vertical plane through the
+    source and the voxel centre, a ray of slope m = dz/drho crosses the voxel's in-plane chord rho_c -+ l_theta/2; the
+    axial factor at that ray's detector row is the fraction of the chord on which the ray is between z_c - dz/2 and
+    z_c + dz/2.  Untilted frame, flat detector (the row coordinate is then linear in m).  The trapezoid joins the
+    exact values at its four vertices by straight lines where the truth is linear in 1/m: a per-cent-level difference
+    at ~20 degrees; a wrong chord length or wrong face heights are tens of per cent."""
+    g = dict(geom3d([0.4], "flat", n=(40, 40, 96), d=(2.0, 2.0, 2.0), nu=128, nv=1600, du=3.0, dv=0.25,
+                    sad=200.0, sdd=400.0), algo="SF-TT")
+    o = Oracle(g)
+    view, ijk = 0, (24, 15, 82)
+    f = o.footprint(view, *ijk)
+    Pc, S = _centre(g, ijk), g["src"][view]
+    e = Pc - S
+    rho_c = math.hypot(e[0], e[1])
+    exy = e[:2] / rho_c
+    l_theta = min(g["dx"] / abs(exy[0]), g["dy"] / abs(exy[1]))
+    t0 = _hit(g, view, S + np.array([exy[0], exy[1], 0.0]))[1]
+    t1 = _hit(g, view, S + np.array([exy[0], exy[1], 1.0]))[1]            # row coordinate of slope 1
+
+    def fraction(t):
+        m = (t - t0) / (t1 - t0)
+        lo, hi = sorted(((Pc[2] - 1.0 - S[2]) / m, (Pc[2] + 1.0 - S[2]) / m))          # dz/2 = 1 mm
+        return max(0.0, min(hi, rho_c + 0.5 * l_theta) - max(lo, rho_c - 0.5 * l_theta)) / l_theta
+
+    sub = (np.arange(8) + 0.5) / 8
+    rows = np.arange(f["l_lo"], f["l_hi"] + 1)
+    brute = np.array([np.mean([fraction((l - 0.5 * g["nv"] + u) * g["dv"]) for u in sub]) for l in rows])
+    assert len(rows) > 20 and brute.max() > 0.99
+    assert np.abs(f["F2"] - brute).max() < 0.02
+    assert abs(f["F2"].sum() / brute.sum() - 1.0) < 5e-3
 
 
 # ---- make_frame's sign flip: u x v pointing AWAY from the detector ------------------------------------------

@@ -93,11 +93,13 @@ def test_cone_beam_fdk_of_a_ball_mid_plane(index, shrink):
     assert np.abs(mid[inside] / MU - 1.0).max() < 4e-2
 
 
-def test_recon_backprojection_weights_are_normalised():
+@pytest.mark.parametrize("algo", ["SF", "SF-TT", "DD"])
+def test_recon_backprojection_weights_are_normalised(algo):
     """R23: with q == 1 and the footprint fully on the detector, B q at a voxel is sum_views d R / a^2
-    exactly (the footprint is a normalised interpolation kernel)."""
+    exactly (the footprint is a normalised interpolation kernel) -- for every voxel model: SF-TT must divide by the
+    AREA of its axial trapezoid (R27), not by its base."""
     c = W.make_config(2, nx=9, ny=9, nz=7, nu=64, nv=64, n_views=5)
-    o = Oracle(W.geom_keys(c))
+    o = Oracle(dict(W.geom_keys(c), algo=algo))
     x = o.bp_recon(np.ones((5, 64, 64)))
     ix, iy, iz = 6, 3, 4
     P = np.array([(ix - 4) * c["dx"], (iy - 4) * c["dy"], (iz - 3) * c["dz"]])
