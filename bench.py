@@ -16,8 +16,9 @@ strong scaling.
 
 roofline.peak is MEASURED in the same run (ct_measure_fp32_peak: FMA-only kernel, before the timed region);
 roofline.achieved = algorithmic flops (FLOP_PER_UPDATE, a count of the method's arithmetic) /
-the dominant kernel's CUDA-event time; the flops the kernels actually execute (ncu op counts) and their DRAM
-traffic are read from profiles/measured_counts.json, which names the capture each number comes from.
+the dominant kernel's CUDA-event time; the flops the kernels actually execute (ncu op counts, packed forms included),
+their DRAM traffic, L2 and shared-memory-pipe utilisation are summed here from the committed ncu capture
+profiles/r3_counts_config<C>.csv (measured_counts); `counts_stale` says whether csrc/ has changed since that capture.
 """
 import argparse
 import json
@@ -59,14 +60,82 @@ def peaks():
     return p
 
 
-def measured_counts(config_index, algo):
-    """ncu-measured per-call counts of the hot kernels (executed fp32 flops, DRAM bytes), from the committed
-    profiles/measured_counts.json; every entry names the capture file it was read from.  None when absent."""
-    try:
-        m = json.load(open(os.path.join(ROOT, "profiles", "measured_counts.json")))
-        return m.get("%s_config%d" % (algo, config_index))
-    except Exception:
+COUNTS_METRICS = (
+    "smsp__sass_thread_inst_executed_op_fadd_pred_on.sum,smsp__sass_thread_inst_executed_op_fmul_pred_on.sum,"
+    "smsp__sass_thread_inst_executed_op_ffma_pred_on.sum,smsp__sass_thread_inst_executed_op_fadd2_pred_on.sum,"
+    "smsp__sass_thread_inst_executed_op_fmul2_pred_on.sum,smsp__sass_thread_inst_executed_op_ffma2_pred_on.sum,"
+    "smsp__thread_inst_executed.sum,smsp__inst_executed.sum,dram__bytes_read.sum,dram__bytes_write.sum,"
+    "gpu__time_duration.sum,l1tex__data_bank_conflicts_pipe_lsu_mem_shared.sum,"
+    "l1tex__data_pipe_lsu_wavefronts_mem_shared.sum,smsp__issue_active.avg.pct_of_peak_sustained_active,"
+    "lts__t_sector_hit_rate.pct,lts__t_sectors.avg.pct_of_peak_sustained_elapsed,"
+    "l1tex__data_pipe_lsu_wavefronts_mem_shared.avg.pct_of_peak_sustained_elapsed")
+COUNTS_CSV = os.path.join(ROOT, "profiles", "r3_counts_config%d.csv")
+COUNTS_STAMP = os.path.join(ROOT, "profiles", "r3_counts_stamp.json")
+CSRC = os.path.join(ROOT, "paper_2503_16741_b200", "csrc")
+
+
+def csrc_sha256():
+    """One hash over the library's sources: says which build a counts capture belongs to."""
+    import hashlib
+    h = hashlib.sha256()
+    for name in sorted(os.listdir(CSRC)):
+        if name.endswith((".cu", ".cuh", ".h", ".cpp")):
+            h.update(name.encode())
+            h.update(open(os.path.join(CSRC, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def measured_counts(config_index, algo, n_updates):
+    """Per-operator-call counts of the hot kernels, summed HERE from the committed ncu capture
+    profiles/r3_counts_config<C>.csv (one `bench.py --steps 1 --warmup 0` run under
+    `ncu --metrics COUNTS_METRICS --clock-control none -k regex:"fp_band|bp_brick|bp_pixel|transpose" --csv`; the full
+    command is in profiles/README.md).  Executed flops = FADD + FMUL + 2 FFMA + 2 (FADD2 + FMUL2) + 4 FFMA2 thread
+    instructions: the packed forms are counted by their own ncu counters (the scalar ones do not see them).
+    Percent-type metrics are time-weighted over the operator's launches.  `stale`: the library's sources differ from
+    the ones the capture was stamped with (`bench.py --stamp-counts`, run when the CSVs are committed).
+    None when there is no capture for this config / voxel model."""
+    import csv
+    path = COUNTS_CSV % config_index
+    if algo != "SF" or not os.path.exists(path):
         return None
+    rows = [l for l in open(path) if l.startswith('"')]
+    launches = {}
+    for r in csv.DictReader(rows):
+        k = launches.setdefault(int(r["ID"]), {"kernel": r["Kernel Name"]})
+        k[r["Metric Name"]] = float(r["Metric Value"].replace(",", ""))
+    ops = {"ct_fp_sf": ("fp_band", "transpose"), "ct_bp_sf": ("bp_brick", "bp_pixel")}
+    out = {}
+    for op, tags in ops.items():
+        ks = [k for k in launches.values() if any(t in k["kernel"] for t in tags)]
+        if not ks:
+            continue
+        tot = lambda m: sum(k.get(m, 0.0) for k in ks)
+        ns = tot("gpu__time_duration.sum")
+        wavg = lambda m: (sum(k[m] * k["gpu__time_duration.sum"] for k in ks) / ns) if ns and all(m in k for k in ks) else None
+        t = lambda o: tot("smsp__sass_thread_inst_executed_op_%s_pred_on.sum" % o)
+        flops = t("fadd") + t("fmul") + 2.0 * t("ffma") + 2.0 * (t("fadd2") + t("fmul2")) + 4.0 * t("ffma2")
+        wf = tot("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum")
+        out[op] = {
+            "launches": len(ks), "ncu_ms": ns / 1e6,
+            "flop_per_update": flops / n_updates,
+            "packed_share_of_flops": (2.0 * (t("fadd2") + t("fmul2")) + 4.0 * t("ffma2")) / flops if flops else None,
+            "thread_inst_per_update": tot("smsp__thread_inst_executed.sum") / n_updates,
+            "dram_bytes": tot("dram__bytes_read.sum") + tot("dram__bytes_write.sum"),
+            "dram_read_bytes": tot("dram__bytes_read.sum"), "dram_write_bytes": tot("dram__bytes_write.sum"),
+            "shared_replay_share": tot("l1tex__data_bank_conflicts_pipe_lsu_mem_shared.sum") / wf if wf else None,
+            "issue_active_pct": wavg("smsp__issue_active.avg.pct_of_peak_sustained_active"),
+            "l2_hit_rate_pct": wavg("lts__t_sector_hit_rate.pct"),
+            "l2_throughput_pct_of_peak": wavg("lts__t_sectors.avg.pct_of_peak_sustained_elapsed"),
+            "shared_pipe_pct_of_peak": wavg("l1tex__data_pipe_lsu_wavefronts_mem_shared.avg.pct_of_peak_sustained_elapsed"),
+            "src": os.path.relpath(path, ROOT),
+        }
+    try:
+        stamp = json.load(open(COUNTS_STAMP))
+    except Exception:
+        stamp = {}
+    out["_stamp"] = stamp
+    out["_stale"] = stamp.get("csrc_sha256") != csrc_sha256()
+    return out
 
 
 class ClockSampler:
@@ -171,6 +240,9 @@ def main():
     ap.add_argument("--impl", default="ctsf")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--stamp-counts", action="store_true",
+                    help="write profiles/r3_counts_stamp.json (hash of csrc/ the committed ncu counts belong to) and exit")
+    ap.add_argument("--print-counts-metrics", action="store_true", help="print the ncu --metrics list of the counts capture")
     ap.add_argument("--algo", default="SF", choices=["SF", "DD", "SF-TT"],
                     help="voxel model: SF (separable footprint, the headline) or DD (distance-driven, row f4)")
     ap.add_argument("--fbp", action="store_true",
@@ -184,6 +256,17 @@ def main():
     c = W.make_config(args.config)
     if args.impl == "reference":
         return run_reference(args, c)
+    if args.print_counts_metrics:
+        print(COUNTS_METRICS)
+        return
+    if args.stamp_counts:
+        # run HERE (in the repository, no GPU needed) when profiles/r3_counts_config*.csv are committed
+        head = subprocess.run(["git", "-C", ROOT, "rev-parse", "--short=12", "HEAD"], capture_output=True, text=True)
+        stamp = {"csrc_sha256": csrc_sha256(), "git_head_at_capture": head.stdout.strip() or None,
+                 "files": sorted(f for f in os.listdir(os.path.join(ROOT, "profiles")) if f.startswith("r3_counts_config"))}
+        json.dump(stamp, open(COUNTS_STAMP, "w"), indent=1)
+        print(json.dumps(stamp))
+        return
 
     import torch
     import torch.distributed as dist
@@ -338,7 +421,7 @@ def main():
         flop = FLOP_PER_UPDATE[args.config] * updates
         alg_bytes = 4.0 * (x.numel() + y.numel())
         dom, dom_ms = ("ct_fp_sf", fp_ms) if fp_ms >= bp_ms else ("ct_bp_sf", bp_ms)
-        mc = measured_counts(args.config, args.algo) or {}
+        mc = (measured_counts(args.config, args.algo, float(W.n_updates(c))) if vs == 1 and not shard_views else None) or {}
         mdom = mc.get(dom, {})
         traffic = mdom.get("dram_bytes") if vs == 1 and not shard_views else None
         achieved = flop / (dom_ms * 1e-3) / 1e12
@@ -377,7 +460,12 @@ def main():
                          "executed_frac": (mdom["flop_per_update"] * updates / (dom_ms * 1e-3) / 1e12 / peak)
                                           if mdom.get("flop_per_update") else None,
                          "issue_slots_busy_pct": mdom.get("issue_active_pct"),
+                         "l2_hit_rate_pct": mdom.get("l2_hit_rate_pct"),
+                         "l2_throughput_pct_of_peak": mdom.get("l2_throughput_pct_of_peak"),
+                         "shared_pipe_pct_of_peak": mdom.get("shared_pipe_pct_of_peak"),
+                         "shared_replay_share": mdom.get("shared_replay_share"),
                          "measured_counts_src": mdom.get("src"),
+                         "counts_stale": mc.get("_stale"), "counts_stamp": mc.get("_stamp"),
                          "hbm": {"algorithmic_bytes": alg_bytes, "achieved_gbs": alg_bytes / (dom_ms * 1e-3) / 1e9,
                                  "peak_gbs": pk["hbm_gbs"], "frac": alg_bytes / (dom_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
                                  "note": "algorithmic bytes / kernel time; the path is ALU-bound by >200x "
